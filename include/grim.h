@@ -1,0 +1,187 @@
+/*
+ * grim.h -- C ABI of the B200-native hot path of grim (arXiv 1702.01106).
+ *
+ * The library advances the primitive variables P of an ideal-GRMHD (N = 8) or extended-GRMHD (N = 10)
+ * fluid by the paper's combined time step + primitive-variable inversion: in every zone, independently,
+ *
+ *     R(P) = [U(P) - U(P_n)]/dt' + div F(P_E) - S = 0                          (eq 19; eq 13)
+ *
+ * is solved by Newton-Raphson (L190-194, eq 20) with a finite-difference Jacobian (L196-216, eqs 21-23), a
+ * dense LU solve with partial pivoting (L198-200, eq 21; L434) and a quadratic backtracking line search
+ * (L218-235, eqs 24-25).  div F comes from slope-limited reconstruction (L154-160) and local Lax-Friedrichs
+ * fluxes (L164-166, eq 17); geometry from eqs 5-8 (L68-89).  "Lnnn" = line of /root/reference/PAPER.md;
+ * "C-n", "G-n" = readings of the paper listed in DESIGN.md.
+ *
+ * Conventions
+ *   - Every array argument is a DEVICE pointer owned by the caller unless its comment says "host".  The library
+ *     never allocates, frees or copies caller arrays to the host.  The context owns geometry tables and scratch.
+ *   - Grid arrays are SoA, fp64: P[v][k][j][i], i (X^1) fastest, ghosts included in every active dimension:
+ *     extent s_d = n_d + 2 ng for d < dim, else n_d (= 1, no ghosts).  Zg = s1*s2*s3 zones per variable.
+ *     Primitive order (L297): rho, u, u~^1, u~^2, u~^3, B^1, B^2, B^3 [, q, dP]   (u~: reading C-9).
+ *   - Flat arrays (grim_invert_primitives, grim_prim_to_conserved) are [v][z], z fastest.
+ *   - All work is enqueued on the stream given at grim_init_grid; calls that return a host scalar
+ *     (n_active_out, dt_used, stats, speeds on host) synchronise that stream, the others are asynchronous.
+ *   - Return value: 0 on success, a negative GRIM_E* code otherwise; grim_last_error() gives the text.  Nothing
+ *     throws across the ABI.  Non-convergence of a zone is NOT an error: it is reported in the per-zone status
+ *     word and in the counts.
+ *   - Arithmetic: fp64, round-to-nearest, no FMA contraction: every + - * / sqrt is a separately rounded IEEE
+ *     operation in a documented order, so results do not depend on launch geometry.
+ *   - There is no CPU fallback: every entry point fails with GRIM_ECUDA if no sm_100 device is usable.
+ */
+#ifndef GRIM_H
+#define GRIM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GRIM_VERSION 100
+
+/* error codes */
+enum { GRIM_OK = 0, GRIM_EINVAL = -1, GRIM_ECUDA = -2, GRIM_ENOMEM = -3, GRIM_ESTATE = -4 };
+
+/* physics model: number of primitives per zone (L297; BASELINE north_star; reading C-1) */
+enum { GRIM_IDEAL = 8, GRIM_EMHD = 10 };
+/* metric (L68-89; C-10) */
+enum { GRIM_MINKOWSKI = 0, GRIM_KERR_MKS = 1 };
+/* reconstruction (L154-160, L115; MP5: C-6) */
+enum { GRIM_MINMOD = 0, GRIM_MP5 = 1 };
+/* Riemann solver (eq 17) */
+enum { GRIM_LLF = 0 };
+/* boundary conditions per direction and side (C-11) */
+enum { GRIM_BC_PERIODIC = 0, GRIM_BC_OUTFLOW = 1, GRIM_BC_REFLECT_POLAR = 2, GRIM_BC_NONE = 3 };
+/* damping time scale tau_R: constant, or r^{3/2} (C-11) */
+enum { GRIM_TAU_CONST = 0, GRIM_TAU_R32 = 1 };
+
+/* per-zone status word */
+enum {
+  GRIM_ST_CONVERGED = 1,     /* ||R||_2 < tol_z                                              (L194) */
+  GRIM_ST_KMAX = 2,          /* stopped at kmax iterations without converging                (L194) */
+  GRIM_ST_LS_EXHAUSTED = 4,  /* some line search used all lsmax+1 trials; last trial taken   (C-14) */
+  GRIM_ST_SINGULAR = 8,      /* zero / non-finite pivot or zero FD step; zone left unchanged (C-17, C-19) */
+  GRIM_ST_NONFINITE = 16     /* non-finite residual norm                                     (C-12) */
+};
+#define GRIM_ST_TERMINAL (GRIM_ST_CONVERGED | GRIM_ST_KMAX | GRIM_ST_SINGULAR | GRIM_ST_NONFINITE)
+
+typedef struct grim_ctx grim_ctx; /* opaque */
+
+typedef struct {
+  int32_t n1, n2, n3;       /* interior zones per direction (unused directions: 1)                 (L406)   */
+  int32_t ng;               /* ghost depth in active directions: >= 2 for minmod, >= 3 for MP5     (G-9)    */
+  int32_t dim;              /* 1, 2 or 3 active directions                                                  */
+  double xstart[3], xend[3];/* extent of the interior in X^i; dX^i = (xend-xstart)/n_i             (L70-72) */
+  int32_t bc[3][2];         /* GRIM_BC_* for [direction][lower, upper]                             (C-11)   */
+  int32_t model;            /* GRIM_IDEAL | GRIM_EMHD                                                       */
+  int32_t recon;            /* GRIM_MINMOD | GRIM_MP5                                                       */
+  double limiter_theta;     /* generalised-minmod theta in [1,2] (L115, L651); also limits EMHD gradients   */
+  int32_t riemann;          /* GRIM_LLF                                                                     */
+  double gamma;             /* adiabatic index                                                     (L248)   */
+  double phi, psi;          /* closure chi = phi cs^2 tau_R, nu = psi cs^2 tau_R                   (L299)   */
+  int32_t tau_mode;         /* GRIM_TAU_CONST | GRIM_TAU_R32                                                */
+  double tau;               /* tau_R when tau_mode == GRIM_TAU_CONST                                        */
+  double fd_eps;            /* epsilon of eq 23 (L202-214; C-16)                                            */
+  double eps_bt;            /* epsilon_BT of the sufficient-decrease test (L223), paper: 1e-4               */
+  double atol, rtol;        /* stop when ||R||_2 < atol + rtol*scale_z (L194; C-2)                          */
+  int32_t kmax, lsmax;      /* Newton-iteration and line-search caps (L194; C-14)                           */
+  double cfl;               /* Courant factor (L651; C-15)                                                  */
+  int32_t device;           /* CUDA device ordinal                                                          */
+  void *stream;             /* cudaStream_t; NULL = the legacy default stream                               */
+} grim_grid_desc;
+
+typedef struct {
+  int64_t zones;              /* interior zones                                                  */
+  int64_t iters_hist[2][16];  /* [stage][min(iterations,15)] number of zones                     */
+  int64_t backtracks[2];      /* rejected line-search trials per stage                           */
+  int64_t unconverged[2];     /* zones without GRIM_ST_CONVERGED per stage                       */
+  double max_resnorm[2];      /* max over zones of ||R||_2 / scale_z per stage                   */
+} grim_step_stats;
+
+/* ---- the six entry points named by the north star ------------------------------------------------------- */
+
+/* Creates a context for one grid (L400-408).  `out` host.  Validates the descriptor (GRIM_EINVAL), selects the
+ * device, allocates scratch: C (N*Zg), G (3*Zg), two P-sized stage buffers, per-zone resnorm/status/iters. */
+int grim_init_grid(grim_ctx **out, const grim_grid_desc *d);
+
+/* Geometry precompute (a0: L68-89 eqs 5-8; L339; C-10): fills the context's tables of g_mu_nu, g^mu^nu,
+ * sqrt(-g), lapse at zone centres and lower face centres, and the connection at centres, on the device.
+ * GRIM_MINKOWSKI: params ignored (geometry is compile-time constant in the kernels).
+ * GRIM_KERR_MKS : params (host) = {a, h}, M = 1; Kerr-Schild transformed by eqs 5-8; X^1 = ln r, X^2 in [0,1].
+ * Must be called before any compute call (GRIM_ESTATE otherwise). */
+int grim_set_metric(grim_ctx *c, int32_t kind, const double *params, int32_t nparams);
+
+/* Steps a1-a3 (L150-173 eqs 17; L99 eq 10; L438): reconstructs P_E to faces, forms LLF fluxes with face-centre
+ * geometry (C-8), and writes the stage constant
+ *     C = -U(P_n)/dt' + div F(P_E) - S^E(P_E)                                  (eq 19 / eq 13; C-5)
+ * and, for EMHD, the three spatial-gradient terms G = (Xq, Xd, divx) of the relaxation targets (eqs 37-38; O-8).
+ * Ghost zones of P_E must be filled (grim_fill_ghosts).  Only interior zones of C, G are written.
+ *   P_E, P_n : N*Zg   C_out : N*Zg or NULL (context scratch)   G_out : 3*Zg or NULL (scratch; ignored for N=8)
+ *   speeds_out : device double[4] or NULL: max over zones of c^d/dX^d (d=1..3) and of sum_d c^d/dX^d (C-15). */
+int grim_compute_fluxes(grim_ctx *c, const double *P_E, const double *P_n, double dt_stage, double *C_out,
+                        double *G_out, double *speeds_out);
+
+/* Steps a4-a7 (L190-235 eqs 20-25): advances the Newton iteration of every interior zone whose status has no
+ * terminal bit by at most `max_iters` iterations (<= 0: until terminal), in place.
+ *   P_n, P_E : N*Zg   C : N*Zg or NULL (scratch of the last grim_compute_fluxes)   G : 3*Zg or NULL (same)
+ *   P_iter : N*Zg, in: P^k, out: P^{k'}     resnorm : Zg, out: ||R(P^{k'})||_2
+ *   status, iters : Zg int32 each, in/out (zero them to start a solve)
+ *   n_active_out : host int64 or NULL: zones still without a terminal bit after the call (synchronises). */
+int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_E, const double *C, const double *G,
+                     double dt_stage, int32_t max_iters, double *P_iter, double *resnorm, int32_t *status,
+                     int32_t *iters, int64_t *n_active_out);
+
+/* Standalone primitive recovery (O-10; BASELINE config 2): for each of nz zones solves
+ * R(P) = (U(P) - U*)/||U*||_2 = 0 by the same Newton iteration, tol = rtol.
+ *   U_target : N*nz flat   geom : NULL (Minkowski) -- curved-space flat inversion is not implemented (GRIM_EINVAL)
+ *   P_inout : N*nz, guess -> result   iters, status : nz int32, out   resnorm : nz, out
+ * Zones are solved to a terminal status; the active set is compacted between iteration sweeps. */
+int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_target, const double *geom, double *P_inout,
+                           int32_t *iters, int32_t *status, double *resnorm);
+
+/* One time step (a8: L113-148, eq 19 then eq 13; O-11): ghost fill, stage 1 (P_E = P_n, dt' = dt/2, guess P_n),
+ * ghost fill, stage 2 (P_E = P_{n+1/2}, dt' = dt, guess P_{n+1/2}); P_inout interior is overwritten by P_{n+1}.
+ *   dt <= 0: dt = cfl / max_z sum_d c^d/dX^d (C-15).   dt_used : host or NULL.   stats : host or NULL
+ * (requesting dt_used or stats synchronises the stream). */
+int grim_timestep(grim_ctx *c, double *P_inout, double dt, double *dt_used, grim_step_stats *stats);
+
+/* ---- helpers beyond the six ------------------------------------------------------------------------------ */
+
+void grim_free(grim_ctx *c);
+const char *grim_last_error(const grim_ctx *c); /* NULL ctx: error of the last failed grim_init_grid */
+int grim_version(void);
+
+/* Padded zone count Zg and padded extents (host out, may be NULL). */
+int64_t grim_zones_padded(const grim_ctx *c, int32_t extents[3]);
+
+/* Ghost fill in place (C-11): direction 1, then 2 (covering direction-1 ghosts), then 3. */
+int grim_fill_ghosts(grim_ctx *c, double *P);
+
+/* U(P) for nz flat zones, Minkowski (eqs 30-32, 39-42); used to build inversion workloads on the device. */
+int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, double *U);
+
+/* Copies the geometry of padded 2-D zone (j,i) -> idx2d = j*s1 + i to the HOST (parity tests of a0):
+ * loc = 0 centre, 1..3 lower face in direction loc.  gcov, gcon: 16 doubles row-major; conn: 64 doubles
+ * [l][m][n] = Gamma^l_{mn} (centre only; may be NULL).  Synchronises. */
+int grim_get_geometry(grim_ctx *c, int32_t loc, int64_t idx2d, double *gcov, double *gcon, double *sqrtmg,
+                      double *alpha, double *tau, double *conn);
+
+/* fp64 pipe probe: runs `iters` dependent-chain-free DFMA (fma=1) or DMUL+DADD (fma=0) instructions per thread
+ * on a full grid and returns fp64 instructions per second (host out).  Used for the ALU roofline denominator. */
+int grim_fp64_probe(grim_ctx *c, int32_t fma, int32_t iters, double *inst_per_s);
+
+/* End-to-end variants taking HOST buffers (pinned or pageable): copy in, run on the device, copy out, on the
+ * context's stream; they return after the stream is synchronised.  Device staging buffers belong to the context.
+ *   grim_timestep_host          : P_host N*Zg in/out; runs nsteps time steps (dt <= 0: chosen per step from cfl).
+ *   grim_invert_primitives_host : U_host, P_host N*nz; iters/status/resnorm host outputs (may be NULL). */
+int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used);
+int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, double *P_host, int32_t *iters_host,
+                                int32_t *status_host, double *resnorm_host);
+
+/* Number of kernels the library has launched on this context since creation (host bookkeeping). */
+int64_t grim_launch_count(const grim_ctx *c);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRIM_H */

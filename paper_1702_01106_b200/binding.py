@@ -1,0 +1,256 @@
+"""ctypes binding of libgrim_b200.so (include/grim.h).  Marshalling only; torch provides device memory/streams.
+
+The `Grid` methods carry the names of the C entry points without the `grim_` prefix.  Tensor arguments must be
+contiguous CUDA tensors of the stated dtype on the grid's device; they are passed as raw device pointers.
+"""
+import ctypes as C
+import os
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+IDEAL, EMHD = 8, 10
+MINKOWSKI, KERR_MKS = 0, 1
+MINMOD, MP5 = 0, 1
+LLF = 0
+BC_PERIODIC, BC_OUTFLOW, BC_REFLECT_POLAR, BC_NONE = 0, 1, 2, 3
+TAU_CONST, TAU_R32 = 0, 1
+ST_CONVERGED, ST_KMAX, ST_LS_EXHAUSTED, ST_SINGULAR, ST_NONFINITE = 1, 2, 4, 8, 16
+ST_TERMINAL = ST_CONVERGED | ST_KMAX | ST_SINGULAR | ST_NONFINITE
+
+
+class GrimError(RuntimeError):
+    pass
+
+
+class GridDesc(C.Structure):
+    _fields_ = [("n1", C.c_int32), ("n2", C.c_int32), ("n3", C.c_int32), ("ng", C.c_int32), ("dim", C.c_int32),
+                ("xstart", C.c_double * 3), ("xend", C.c_double * 3), ("bc", (C.c_int32 * 2) * 3),
+                ("model", C.c_int32), ("recon", C.c_int32), ("limiter_theta", C.c_double), ("riemann", C.c_int32),
+                ("gamma", C.c_double), ("phi", C.c_double), ("psi", C.c_double),
+                ("tau_mode", C.c_int32), ("tau", C.c_double),
+                ("fd_eps", C.c_double), ("eps_bt", C.c_double), ("atol", C.c_double), ("rtol", C.c_double),
+                ("kmax", C.c_int32), ("lsmax", C.c_int32), ("cfl", C.c_double),
+                ("device", C.c_int32), ("stream", C.c_void_p)]
+
+
+class StepStats(C.Structure):
+    _fields_ = [("zones", C.c_int64), ("iters_hist", (C.c_int64 * 16) * 2), ("backtracks", C.c_int64 * 2),
+                ("unconverged", C.c_int64 * 2), ("max_resnorm", C.c_double * 2)]
+
+
+_vp, _dbl, _i32, _i64 = C.c_void_p, C.c_double, C.c_int32, C.c_int64
+_pd, _pi32, _pi64 = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+
+# name -> (restype, argtypes): every symbol include/grim.h declares
+_SIGNATURES = {
+    "grim_init_grid": (C.c_int, [C.POINTER(_vp), C.POINTER(GridDesc)]),
+    "grim_set_metric": (C.c_int, [_vp, _i32, _pd, _i32]),
+    "grim_compute_fluxes": (C.c_int, [_vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
+    "grim_newton_step": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _i32, _vp, _vp, _vp, _vp, _pi64]),
+    "grim_invert_primitives": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "grim_timestep": (C.c_int, [_vp, _vp, _dbl, _pd, C.POINTER(StepStats)]),
+    "grim_free": (None, [_vp]),
+    "grim_last_error": (C.c_char_p, [_vp]),
+    "grim_version": (C.c_int, []),
+    "grim_zones_padded": (_i64, [_vp, _pi32]),
+    "grim_fill_ghosts": (C.c_int, [_vp, _vp]),
+    "grim_prim_to_conserved": (C.c_int, [_vp, _i64, _vp, _vp]),
+    "grim_get_geometry": (C.c_int, [_vp, _i32, _i64, _pd, _pd, _pd, _pd, _pd, _pd]),
+    "grim_fp64_probe": (C.c_int, [_vp, _i32, _i32, _pd]),
+    "grim_timestep_host": (C.c_int, [_vp, _vp, _i32, _dbl, _pd]),
+    "grim_invert_primitives_host": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp]),
+    "grim_launch_count": (_i64, [_vp]),
+}
+
+
+def exported_symbols():
+    return sorted(_SIGNATURES)
+
+
+def lib_path():
+    return os.path.join(HERE, "libgrim_b200.so")
+
+
+_lib = None
+
+
+def lib():
+    """Loads the CUDA library.  No fallback: a missing library is an error."""
+    global _lib
+    if _lib is None:
+        p = lib_path()
+        if not os.path.exists(p):
+            raise GrimError("%s is missing: build it with `python -m paper_1702_01106_b200.build` "
+                            "(there is no CPU fallback)" % p)
+        L = C.CDLL(p)
+        for name, (res, args) in _SIGNATURES.items():
+            f = getattr(L, name)
+            f.restype = res
+            f.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _ptr(t, dtype=None):
+    """Raw device pointer of a contiguous CUDA tensor (None -> NULL)."""
+    if t is None:
+        return None
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous()):
+        raise GrimError("expected a contiguous CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise GrimError("expected dtype %s, got %s" % (dtype, t.dtype))
+    return C.c_void_p(t.data_ptr())
+
+
+def _host_ptr(t, dtype=None):
+    import torch
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.is_contiguous()):
+        raise GrimError("expected a contiguous host tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise GrimError("expected dtype %s, got %s" % (dtype, t.dtype))
+    return C.c_void_p(t.data_ptr())
+
+
+class Grid:
+    """Owns a grim_ctx.  Grid arrays are torch.float64 CUDA tensors of shape [nvar, s3, s2, s1]."""
+
+    def __init__(self, n1, n2=1, n3=1, ng=3, dim=2, xstart=(0.0, 0.0, 0.0), xend=(1.0, 1.0, 1.0), bc=BC_PERIODIC,
+                 model=EMHD, recon=MINMOD, limiter_theta=1.0, gamma=4.0 / 3.0, phi=1.0, psi=1.0, tau_mode=TAU_CONST,
+                 tau=1.0, fd_eps=4e-8, eps_bt=1e-4, atol=0.0, rtol=1e-14, kmax=8, lsmax=5, cfl=0.5,
+                 metric=MINKOWSKI, metric_params=(), device=0, stream=None):
+        import torch
+        self.torch = torch
+        d = GridDesc()
+        d.n1, d.n2, d.n3, d.ng, d.dim = n1, n2, n3, ng, dim
+        for a in range(3):
+            d.xstart[a], d.xend[a] = float(xstart[a]), float(xend[a])
+            for s in range(2):
+                d.bc[a][s] = bc if isinstance(bc, int) else bc[a][s]
+        d.model, d.recon, d.limiter_theta, d.riemann = model, recon, limiter_theta, LLF
+        d.gamma, d.phi, d.psi, d.tau_mode, d.tau = gamma, phi, psi, tau_mode, tau
+        d.fd_eps, d.eps_bt, d.atol, d.rtol, d.kmax, d.lsmax, d.cfl = fd_eps, eps_bt, atol, rtol, kmax, lsmax, cfl
+        d.device = device
+        if stream is None and torch.cuda.is_available():
+            stream = torch.cuda.current_stream(device).cuda_stream
+        d.stream = stream
+        self.desc = d
+        self.h = _vp()
+        self._L = lib()
+        rc = self._L.grim_init_grid(C.byref(self.h), C.byref(d))
+        if rc != 0:
+            msg = self._L.grim_last_error(None)
+            self.h = None
+            raise GrimError("grim_init_grid failed (%d): %s" % (rc, msg.decode() if msg else ""))
+        self.device = torch.device("cuda", device)
+        self.nvar = model
+        self.n = (n1, n2, n3)
+        self.ngd = tuple(ng if a < dim else 0 for a in range(3))
+        self.sz = tuple(self.n[a] + 2 * self.ngd[a] for a in range(3))
+        self.shape = (model, self.sz[2], self.sz[1], self.sz[0])
+        self.zg = self.sz[0] * self.sz[1] * self.sz[2]
+        self.zones = n1 * n2 * n3
+        self.set_metric(metric, metric_params)
+
+    # -- plumbing ------------------------------------------------------------------------------------------
+    def _check(self, rc, what):
+        if rc != 0:
+            msg = self._L.grim_last_error(self.h)
+            raise GrimError("%s failed (%d): %s" % (what, rc, msg.decode() if msg else ""))
+
+    def close(self):
+        if getattr(self, "h", None):
+            self._L.grim_free(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def zeros(self, nvar=None, dtype=None):
+        t = self.torch
+        shape = ((nvar,) if nvar else ()) + self.shape[1:]
+        return t.zeros(shape, dtype=dtype or t.float64, device=self.device)
+
+    def interior(self, A):
+        g = self.ngd
+        return A[..., g[2]:g[2] + self.n[2], g[1]:g[1] + self.n[1], g[0]:g[0] + self.n[0]]
+
+    def launch_count(self):
+        return int(self._L.grim_launch_count(self.h))
+
+    # -- the entry points ----------------------------------------------------------------------------------
+    def set_metric(self, kind, params=()):
+        arr = (C.c_double * max(len(params), 1))(*[float(x) for x in params])
+        self._check(self._L.grim_set_metric(self.h, kind, arr, len(params)), "grim_set_metric")
+
+    def fill_ghosts(self, P):
+        self._check(self._L.grim_fill_ghosts(self.h, _ptr(P, self.torch.float64)), "grim_fill_ghosts")
+
+    def compute_fluxes(self, P_E, P_n, dt_stage, C_out=None, G_out=None, speeds_out=None):
+        f64 = self.torch.float64
+        self._check(self._L.grim_compute_fluxes(self.h, _ptr(P_E, f64), _ptr(P_n, f64), dt_stage, _ptr(C_out, f64),
+                                                _ptr(G_out, f64), _ptr(speeds_out, f64)), "grim_compute_fluxes")
+
+    def newton_step(self, P_n, P_E, C_, G_, dt_stage, max_iters, P_iter, resnorm, status, iters, want_active=True):
+        t = self.torch
+        na = C.c_int64(0)
+        self._check(self._L.grim_newton_step(self.h, _ptr(P_n, t.float64), _ptr(P_E, t.float64), _ptr(C_, t.float64),
+                                             _ptr(G_, t.float64), dt_stage, max_iters, _ptr(P_iter, t.float64),
+                                             _ptr(resnorm, t.float64), _ptr(status, t.int32), _ptr(iters, t.int32),
+                                             C.byref(na) if want_active else None), "grim_newton_step")
+        return na.value if want_active else None
+
+    def invert_primitives(self, U_target, P_inout, iters, status, resnorm):
+        t = self.torch
+        nz = P_inout.shape[1]
+        self._check(self._L.grim_invert_primitives(self.h, nz, _ptr(U_target, t.float64), None,
+                                                   _ptr(P_inout, t.float64), _ptr(iters, t.int32),
+                                                   _ptr(status, t.int32), _ptr(resnorm, t.float64)),
+                    "grim_invert_primitives")
+
+    def invert_primitives_host(self, U_host, P_host, iters_host=None, status_host=None, resnorm_host=None):
+        t = self.torch
+        nz = P_host.shape[1]
+        self._check(self._L.grim_invert_primitives_host(self.h, nz, _host_ptr(U_host, t.float64),
+                                                        _host_ptr(P_host, t.float64), _host_ptr(iters_host, t.int32),
+                                                        _host_ptr(status_host, t.int32),
+                                                        _host_ptr(resnorm_host, t.float64)),
+                    "grim_invert_primitives_host")
+
+    def prim_to_conserved(self, P, U):
+        t = self.torch
+        self._check(self._L.grim_prim_to_conserved(self.h, P.shape[1], _ptr(P, t.float64), _ptr(U, t.float64)),
+                    "grim_prim_to_conserved")
+
+    def timestep(self, P, dt=0.0, want_dt=False, want_stats=False):
+        """One time step in place.  Returns (dt_used or None, StepStats or None)."""
+        dtu = C.c_double(0.0)
+        st = StepStats()
+        self._check(self._L.grim_timestep(self.h, _ptr(P, self.torch.float64), dt, C.byref(dtu) if want_dt else None,
+                                          C.byref(st) if want_stats else None), "grim_timestep")
+        return (dtu.value if want_dt else None), (st if want_stats else None)
+
+    def timestep_host(self, P_host, nsteps, dt=0.0):
+        dtu = C.c_double(0.0)
+        self._check(self._L.grim_timestep_host(self.h, _host_ptr(P_host, self.torch.float64), nsteps, dt,
+                                               C.byref(dtu)), "grim_timestep_host")
+        return dtu.value
+
+    def get_geometry(self, loc, j, i):
+        import numpy as np
+        gcov, gcon, conn = np.zeros(16), np.zeros(16), np.zeros(64)
+        sg, al, tau = C.c_double(), C.c_double(), C.c_double()
+        dp = lambda a: a.ctypes.data_as(_pd)  # noqa: E731
+        self._check(self._L.grim_get_geometry(self.h, loc, j * self.sz[0] + i, dp(gcov), dp(gcon), C.byref(sg),
+                                              C.byref(al), C.byref(tau), dp(conn)), "grim_get_geometry")
+        return gcov.reshape(4, 4), gcon.reshape(4, 4), sg.value, al.value, tau.value, conn.reshape(4, 4, 4)
+
+    def fp64_probe(self, fma=True, iters=1 << 16):
+        out = C.c_double(0.0)
+        self._check(self._L.grim_fp64_probe(self.h, 1 if fma else 0, iters, C.byref(out)), "grim_fp64_probe")
+        return out.value

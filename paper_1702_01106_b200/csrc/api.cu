@@ -1,0 +1,480 @@
+// api.cu -- the C ABI of include/grim.h: context, argument checking, stage sequencing.  Host code only; every
+// step of the hot path runs in the kernels of kernels_*.cu.
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdio.h>
+#include <string.h>
+
+#include <string>
+
+#include "../../include/grim.h"
+#include "grim_internal.h"
+
+using namespace grim;
+
+struct grim_ctx {
+  grim_grid_desc d;
+  GridView gv;
+  cudaStream_t stream;
+  int metric_set;
+  // geometry tables
+  double *geomC, *geomF[3], *conn;
+  // scratch
+  double *C, *G;               // stage constant, EMHD gradient terms
+  double *Fface, *cface;       // face fluxes (3 x N x Zg), face speeds (3 x Zg)
+  double *Ph, *Pnew;           // stage buffers
+  double *resnorm;
+  int32_t *status, *iters;
+  Counters *cnt;               // device
+  StatsDev *stats;             // device, 2 stages
+  double *probe_sink;
+  long long *list[2];          // inversion active lists
+  long long list_cap;
+  double *hostP;               // staging for the *_host entry points
+  double *invbuf;              // U, P, resnorm, iters, status of grim_invert_primitives_host
+  long long invbuf_nz;
+  int64_t launches;
+  std::string err;
+};
+
+static std::string g_init_error;
+
+static int fail(grim_ctx *c, int code, const std::string &msg) {
+  if (c) c->err = msg;
+  else g_init_error = msg;
+  return code;
+}
+
+#define CU(call)                                                                                       \
+  do {                                                                                                 \
+    cudaError_t e_ = (call);                                                                           \
+    if (e_ != cudaSuccess)                                                                             \
+      return fail(c, e_ == cudaErrorMemoryAllocation ? GRIM_ENOMEM : GRIM_ECUDA,                       \
+                  std::string(#call) + ": " + cudaGetErrorString(e_));                                 \
+  } while (0)
+
+static int check_launch(grim_ctx *c, const char *what) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(c, GRIM_ECUDA, std::string(what) + ": " + cudaGetErrorString(e));
+  return GRIM_OK;
+}
+
+extern "C" int grim_version(void) { return GRIM_VERSION; }
+
+extern "C" const char *grim_last_error(const grim_ctx *c) { return c ? c->err.c_str() : g_init_error.c_str(); }
+
+extern "C" int64_t grim_launch_count(const grim_ctx *c) { return c ? c->launches : 0; }
+
+extern "C" int64_t grim_zones_padded(const grim_ctx *c, int32_t extents[3]) {
+  if (!c) return 0;
+  if (extents)
+    for (int a = 0; a < 3; a++) extents[a] = c->gv.sz[a];
+  return c->gv.zg;
+}
+
+extern "C" void grim_free(grim_ctx *c) {
+  if (!c) return;
+  cudaSetDevice(c->d.device);
+  cudaStreamSynchronize(c->stream);
+  void *ptrs[] = {c->geomC, c->geomF[0], c->geomF[1], c->geomF[2], c->conn, c->C, c->G, c->Fface, c->cface,
+                  c->Ph, c->Pnew, c->resnorm, c->status, c->iters, c->cnt, c->stats, c->probe_sink,
+                  c->list[0], c->list[1], c->hostP, c->invbuf};
+  for (void *p : ptrs)
+    if (p) cudaFree(p);
+  delete c;
+}
+
+extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
+  grim_ctx *c = nullptr;
+  if (!out || !d) return fail(c, GRIM_EINVAL, "grim_init_grid: null argument");
+  *out = nullptr;
+  if (d->dim < 1 || d->dim > 3) return fail(c, GRIM_EINVAL, "dim must be 1, 2 or 3");
+  if (d->model != GRIM_IDEAL && d->model != GRIM_EMHD) return fail(c, GRIM_EINVAL, "model must be 8 or 10");
+  if (d->recon != GRIM_MINMOD && d->recon != GRIM_MP5) return fail(c, GRIM_EINVAL, "unknown reconstruction");
+  if (d->riemann != GRIM_LLF) return fail(c, GRIM_EINVAL, "only the LLF flux (eq 17) is implemented");
+  const int nn[3] = {d->n1, d->n2, d->n3};
+  const int need = d->recon == GRIM_MP5 ? 3 : 2;
+  if (d->ng < need) return fail(c, GRIM_EINVAL, "ghost depth too small for the reconstruction");
+  for (int a = 0; a < 3; a++) {
+    if (nn[a] < 1) return fail(c, GRIM_EINVAL, "zone counts must be positive");
+    if (a >= d->dim && nn[a] != 1) return fail(c, GRIM_EINVAL, "inactive directions must have one zone");
+    if (a < d->dim && nn[a] < d->ng) return fail(c, GRIM_EINVAL, "active directions need at least ng zones");
+    if (a < d->dim && !(d->xend[a] > d->xstart[a])) return fail(c, GRIM_EINVAL, "empty coordinate extent");
+    for (int s = 0; s < 2; s++)
+      if (d->bc[a][s] < 0 || d->bc[a][s] > 3) return fail(c, GRIM_EINVAL, "unknown boundary condition");
+  }
+  if (!(d->gamma > 1.0)) return fail(c, GRIM_EINVAL, "adiabatic index must exceed 1");
+  if (!(d->limiter_theta >= 1.0 && d->limiter_theta <= 2.0)) return fail(c, GRIM_EINVAL, "limiter_theta outside [1,2]");
+  if (!(d->fd_eps > 0.0) || d->kmax < 0 || d->lsmax < 0) return fail(c, GRIM_EINVAL, "bad solver parameters");
+  if (d->model == GRIM_EMHD && !(d->tau_mode == GRIM_TAU_R32 || d->tau > 0.0))
+    return fail(c, GRIM_EINVAL, "tau_R must be positive");
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return fail(c, GRIM_ECUDA, "no CUDA device: this library has no CPU fallback");
+  if (d->device < 0 || d->device >= ndev) return fail(c, GRIM_EINVAL, "device ordinal out of range");
+  if (cudaSetDevice(d->device) != cudaSuccess) return fail(c, GRIM_ECUDA, "cudaSetDevice failed");
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, d->device) != cudaSuccess) return fail(c, GRIM_ECUDA, "no device properties");
+  if (prop.major != 10) return fail(c, GRIM_ECUDA, "kernels are built for sm_100a only");
+
+  c = new grim_ctx();
+  c->d = *d;
+  c->stream = (cudaStream_t)d->stream;
+  c->metric_set = 0;
+  c->launches = 0;
+  GridView &gv = c->gv;
+  memset(&gv, 0, sizeof(gv));
+  gv.dim = d->dim;
+  gv.nvar = d->model;
+  gv.recon = d->recon;
+  gv.metric = -1;
+  gv.nint = 1;
+  gv.zg = 1;
+  for (int a = 0; a < 3; a++) {
+    gv.n[a] = nn[a];
+    gv.ngd[a] = (a < d->dim) ? d->ng : 0;
+    gv.sz[a] = gv.n[a] + 2 * gv.ngd[a];
+    gv.dx[a] = (d->xend[a] - d->xstart[a]) / gv.n[a];  // L70
+    gv.idx[a] = 1.0 / gv.dx[a];
+    gv.xstart[a] = d->xstart[a];
+    gv.nint *= gv.n[a];
+    gv.zg *= gv.sz[a];
+  }
+  gv.n2d = (long long)gv.sz[0] * gv.sz[1];
+  gv.theta = d->limiter_theta;
+  gv.m.gam = d->gamma;
+  gv.m.gm1 = d->gamma - 1.0;
+  gv.m.phi = d->phi;
+  gv.m.psi = d->psi;
+  gv.tau_const = d->tau;
+  gv.sp.fd_eps = d->fd_eps;
+  gv.sp.eps_bt = d->eps_bt;
+  gv.sp.atol = d->atol;
+  gv.sp.rtol = d->rtol;
+  gv.sp.kmax = d->kmax;
+  gv.sp.lsmax = d->lsmax;
+
+  const size_t N = (size_t)gv.nvar, zg = (size_t)gv.zg, n2d = (size_t)gv.n2d;
+  auto alloc = [&](void **p, size_t bytes) { return cudaMalloc(p, bytes ? bytes : 8); };
+  cudaError_t e = cudaSuccess;
+#define A_(ptr, bytes) if (e == cudaSuccess) e = alloc((void **)&(ptr), (bytes))
+  A_(c->geomC, GT_NCOMP * n2d * 8);
+  for (int a = 0; a < 3; a++) A_(c->geomF[a], GT_NCOMP * n2d * 8);
+  A_(c->conn, CONN_NCOMP * n2d * 8);
+  A_(c->C, N * zg * 8);
+  A_(c->G, 3 * zg * 8);
+  A_(c->Fface, 3 * N * zg * 8);
+  A_(c->cface, 3 * zg * 8);
+  A_(c->Ph, N * zg * 8);
+  A_(c->Pnew, N * zg * 8);
+  A_(c->resnorm, zg * 8);
+  A_(c->status, zg * 4);
+  A_(c->iters, zg * 4);
+  A_(c->cnt, sizeof(Counters));
+  A_(c->stats, 2 * sizeof(StatsDev));
+  A_(c->probe_sink, 64);
+#undef A_
+  if (e != cudaSuccess) {
+    std::string msg = std::string("cudaMalloc: ") + cudaGetErrorString(e);
+    grim_free(c);
+    return fail(nullptr, GRIM_ENOMEM, msg);
+  }
+  gv.geomC = c->geomC;
+  for (int a = 0; a < 3; a++) gv.geomF[a] = c->geomF[a];
+  gv.conn = c->conn;
+  cudaMemsetAsync(c->G, 0, 3 * zg * 8, c->stream);
+  cudaMemsetAsync(c->C, 0, N * zg * 8, c->stream);
+  *out = c;
+  return GRIM_OK;
+}
+
+extern "C" int grim_set_metric(grim_ctx *c, int32_t kind, const double *params, int32_t nparams) {
+  if (!c) return GRIM_EINVAL;
+  CU(cudaSetDevice(c->d.device));
+  if (kind == GRIM_MINKOWSKI) {
+    c->launches += launch_metric_flat(c->gv, c->geomC, c->geomF[0], c->geomF[1], c->geomF[2], c->conn, c->stream);
+  } else if (kind == GRIM_KERR_MKS) {
+    if (!params || nparams < 2) return fail(c, GRIM_EINVAL, "Kerr needs params = {a, h}");
+    if (c->d.dim < 2) return fail(c, GRIM_EINVAL, "Kerr needs at least the X1, X2 directions");
+    c->launches += launch_metric_kerr(c->gv, params[0], params[1], c->d.tau_mode, c->geomC, c->geomF[0],
+                                      c->geomF[1], c->geomF[2], c->conn, c->stream);
+  } else {
+    return fail(c, GRIM_EINVAL, "unknown metric");
+  }
+  int rc = check_launch(c, "metric kernel");
+  if (rc) return rc;
+  c->gv.metric = kind;
+  c->metric_set = 1;
+  return GRIM_OK;
+}
+
+static int need_metric(grim_ctx *c) {
+  if (!c) return GRIM_EINVAL;
+  if (!c->metric_set) return fail(c, GRIM_ESTATE, "grim_set_metric has not been called");
+  return GRIM_OK;
+}
+
+extern "C" int grim_fill_ghosts(grim_ctx *c, double *P) {
+  if (!c || !P) return fail(c, GRIM_EINVAL, "grim_fill_ghosts: null argument");
+  CU(cudaSetDevice(c->d.device));
+  c->launches += launch_fill_ghosts(c->gv, c->d.bc, P, c->stream);
+  return check_launch(c, "fill_ghosts kernel");
+}
+
+extern "C" int grim_compute_fluxes(grim_ctx *c, const double *P_E, const double *P_n, double dt_stage,
+                                   double *C_out, double *G_out, double *speeds_out) {
+  int rc = need_metric(c);
+  if (rc) return rc;
+  if (!P_E || !P_n) return fail(c, GRIM_EINVAL, "grim_compute_fluxes: null P_E or P_n");
+  if (!(dt_stage > 0.0)) return fail(c, GRIM_EINVAL, "dt_stage must be positive");
+  CU(cudaSetDevice(c->d.device));
+  Counters *cnt = nullptr;
+  if (speeds_out) {
+    CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
+    cnt = c->cnt;
+  }
+  c->launches += launch_fluxes(c->gv, P_E, P_n, dt_stage, C_out ? C_out : c->C, G_out ? G_out : c->G, c->Fface,
+                               c->cface, cnt, c->stream);
+  rc = check_launch(c, "flux kernels");
+  if (rc) return rc;
+  if (speeds_out)
+    CU(cudaMemcpyAsync(speeds_out, c->cnt->speeds, 4 * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  return GRIM_OK;
+}
+
+extern "C" int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_E, const double *C, const double *G,
+                                double dt_stage, int32_t max_iters, double *P_iter, double *resnorm,
+                                int32_t *status, int32_t *iters, int64_t *n_active_out) {
+  int rc = need_metric(c);
+  if (rc) return rc;
+  if (!P_n || !P_E || !P_iter || !resnorm || !status || !iters)
+    return fail(c, GRIM_EINVAL, "grim_newton_step: null array argument");
+  if (!(dt_stage > 0.0)) return fail(c, GRIM_EINVAL, "dt_stage must be positive");
+  CU(cudaSetDevice(c->d.device));
+  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
+  c->launches += launch_newton_stage(c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, dt_stage, max_iters, P_iter,
+                                     resnorm, status, iters, c->cnt, c->stream);
+  rc = check_launch(c, "newton_stage kernel");
+  if (rc) return rc;
+  if (n_active_out) {
+    unsigned long long na = 0;
+    CU(cudaMemcpyAsync(&na, &c->cnt->n_active, sizeof(na), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    *n_active_out = (int64_t)na;
+  }
+  return GRIM_OK;
+}
+
+extern "C" int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, double *U) {
+  if (!c || !P || !U || nz < 0) return fail(c, GRIM_EINVAL, "grim_prim_to_conserved: bad argument");
+  CU(cudaSetDevice(c->d.device));
+  c->launches += launch_prim_to_conserved(c->gv, nz, P, U, c->stream);
+  return check_launch(c, "prim_to_conserved kernel");
+}
+
+extern "C" int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_target, const double *geom,
+                                      double *P_inout, int32_t *iters, int32_t *status, double *resnorm) {
+  if (!c) return GRIM_EINVAL;
+  if (geom) return fail(c, GRIM_EINVAL, "curved-space flat inversion is not implemented; pass geom = NULL");
+  if (nz < 0 || (nz > 0 && (!U_target || !P_inout || !iters || !status || !resnorm)))
+    return fail(c, GRIM_EINVAL, "grim_invert_primitives: bad argument");
+  if (nz == 0) return GRIM_OK;
+  CU(cudaSetDevice(c->d.device));
+  if (c->list_cap < nz) {
+    for (int a = 0; a < 2; a++) {
+      if (c->list[a]) cudaFree(c->list[a]);
+      c->list[a] = nullptr;
+      CU(cudaMalloc((void **)&c->list[a], (size_t)nz * sizeof(long long)));
+    }
+    c->list_cap = nz;
+  }
+  // sweeps of a few iterations each over the compacted set of zones that are still iterating
+  const int kmax = c->gv.sp.kmax;
+  long long nlist = nz;
+  int first = 1, cur = 0, done_iters = 0;
+  while (nlist > 0) {
+    const int sweep = first ? 4 : 2;
+    CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
+    c->launches += launch_invert(c->gv, nz, nlist, c->list[cur], U_target, P_inout, iters, status, resnorm, sweep,
+                                 first, c->list[cur ^ 1], c->cnt, c->stream);
+    int rc = check_launch(c, "invert kernel");
+    if (rc) return rc;
+    unsigned long long cntn = 0;
+    CU(cudaMemcpyAsync(&cntn, &c->cnt->list_count, sizeof(cntn), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    nlist = (long long)cntn;
+    cur ^= 1;
+    first = 0;
+    done_iters += sweep;
+    if (done_iters > kmax + 8) break;  // cannot happen: every zone reaches kmax
+  }
+  return GRIM_OK;
+}
+
+static void stats_to_host(const StatsDev *h, int stage, grim_step_stats *st) {
+  for (int b = 0; b < 16; b++) st->iters_hist[stage][b] = (int64_t)h->hist[b];
+  st->unconverged[stage] = (int64_t)h->unconverged;
+  double v;
+  memcpy(&v, &h->max_rel, sizeof(v));
+  st->max_resnorm[stage] = v;
+}
+
+extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used, grim_step_stats *stats) {
+  int rc = need_metric(c);
+  if (rc) return rc;
+  if (!P) return fail(c, GRIM_EINVAL, "grim_timestep: null P");
+  CU(cudaSetDevice(c->d.device));
+  const GridView &gv = c->gv;
+  const size_t pbytes = (size_t)gv.nvar * gv.zg * 8;
+  cudaStream_t s = c->stream;
+  unsigned long long bt[2] = {0, 0};
+
+  c->launches += launch_fill_ghosts(gv, c->d.bc, P, s);
+  if (!(dt > 0.0)) {
+    // C-15: dt = cfl / max_z sum_d c^d/dX^d, from a flux pass over P_n
+    CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
+    c->launches += launch_fluxes(gv, P, P, 1.0, c->C, c->G, c->Fface, c->cface, c->cnt, s);
+    double sp3 = 0.0;
+    CU(cudaMemcpyAsync(&sp3, &c->cnt->speeds[3], sizeof(double), cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    if (!(sp3 > 0.0)) return fail(c, GRIM_ESTATE, "maximum wave speed is not positive");
+    dt = c->d.cfl / sp3;
+  }
+  if (stats) CU(cudaMemsetAsync(c->stats, 0, 2 * sizeof(StatsDev), s));
+
+  // stage 1: P_E = P_n, dt' = dt/2, guess P_n (eq 19; C-7)
+  const double dt1 = 0.5 * dt;
+  c->launches += launch_fluxes(gv, P, P, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s);
+  CU(cudaMemcpyAsync(c->Ph, P, pbytes, cudaMemcpyDeviceToDevice, s));
+  CU(cudaMemsetAsync(c->status, 0, (size_t)gv.zg * 4, s));
+  CU(cudaMemsetAsync(c->iters, 0, (size_t)gv.zg * 4, s));
+  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
+  c->launches += launch_newton_stage(gv, P, P, c->C, c->G, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s);
+  if (stats) {
+    c->launches += launch_stats(gv, P, dt1, c->resnorm, c->status, c->iters, &c->stats[0], s);
+    CU(cudaMemcpyAsync(&bt[0], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));
+  }
+  // stage 2: P_E = P_{n+1/2}, dt' = dt, guess P_{n+1/2} (eq 13)
+  c->launches += launch_fill_ghosts(gv, c->d.bc, c->Ph, s);
+  c->launches += launch_fluxes(gv, c->Ph, P, dt, c->C, c->G, c->Fface, c->cface, nullptr, s);
+  CU(cudaMemcpyAsync(c->Pnew, c->Ph, pbytes, cudaMemcpyDeviceToDevice, s));
+  CU(cudaMemsetAsync(c->status, 0, (size_t)gv.zg * 4, s));
+  CU(cudaMemsetAsync(c->iters, 0, (size_t)gv.zg * 4, s));
+  if (stats) CU(cudaStreamSynchronize(s));  // bt[0] must land before the counters are cleared
+  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
+  c->launches += launch_newton_stage(gv, P, c->Ph, c->C, c->G, dt, 0, c->Pnew, c->resnorm, c->status, c->iters,
+                                     c->cnt, s);
+  if (stats) {
+    c->launches += launch_stats(gv, P, dt, c->resnorm, c->status, c->iters, &c->stats[1], s);
+    CU(cudaMemcpyAsync(&bt[1], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));
+  }
+  CU(cudaMemcpyAsync(P, c->Pnew, pbytes, cudaMemcpyDeviceToDevice, s));
+  rc = check_launch(c, "timestep kernels");
+  if (rc) return rc;
+  if (stats) {
+    StatsDev h[2];
+    CU(cudaMemcpyAsync(h, c->stats, sizeof(h), cudaMemcpyDeviceToHost, s));
+    CU(cudaStreamSynchronize(s));
+    memset(stats, 0, sizeof(*stats));
+    stats->zones = gv.nint;
+    stats_to_host(&h[0], 0, stats);
+    stats_to_host(&h[1], 1, stats);
+    stats->backtracks[0] = (int64_t)bt[0];
+    stats->backtracks[1] = (int64_t)bt[1];
+  }
+  if (dt_used) {
+    CU(cudaStreamSynchronize(s));
+    *dt_used = dt;
+  }
+  return GRIM_OK;
+}
+
+extern "C" int grim_get_geometry(grim_ctx *c, int32_t loc, int64_t idx2d, double *gcov, double *gcon,
+                                 double *sqrtmg, double *alpha, double *tau, double *conn) {
+  int rc = need_metric(c);
+  if (rc) return rc;
+  if (loc < 0 || loc > 3 || idx2d < 0 || idx2d >= c->gv.n2d) return fail(c, GRIM_EINVAL, "bad location");
+  CU(cudaSetDevice(c->d.device));
+  const double *tab = loc == 0 ? c->geomC : c->geomF[loc - 1];
+  double comp[GT_NCOMP];
+  CU(cudaStreamSynchronize(c->stream));
+  CU(cudaMemcpy2D(comp, 8, tab + idx2d, (size_t)c->gv.n2d * 8, 8, GT_NCOMP, cudaMemcpyDeviceToHost));
+  for (int m = 0; m < 4; m++)
+    for (int n = 0; n < 4; n++) {
+      if (gcov) gcov[m * 4 + n] = comp[GT_GCOV + sym4(m, n)];
+      if (gcon) gcon[m * 4 + n] = comp[GT_GCON + sym4(m, n)];
+    }
+  if (sqrtmg) *sqrtmg = comp[GT_SQRTMG];
+  if (alpha) *alpha = comp[GT_ALPHA];
+  if (tau) *tau = comp[GT_TAU];
+  if (conn) CU(cudaMemcpy2D(conn, 8, c->conn + idx2d, (size_t)c->gv.n2d * 8, 8, CONN_NCOMP, cudaMemcpyDeviceToHost));
+  return GRIM_OK;
+}
+
+extern "C" int grim_fp64_probe(grim_ctx *c, int32_t fma, int32_t iters, double *inst_per_s) {
+  if (!c || !inst_per_s || iters <= 0) return fail(c, GRIM_EINVAL, "grim_fp64_probe: bad argument");
+  CU(cudaSetDevice(c->d.device));
+  cudaDeviceProp prop;
+  CU(cudaGetDeviceProperties(&prop, c->d.device));
+  const int threads = 256, blocks = prop.multiProcessorCount * 8;
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  launch_fp64_probe(fma, iters, c->probe_sink, blocks, threads, c->stream);  // warm-up
+  CU(cudaEventRecord(e0, c->stream));
+  launch_fp64_probe(fma, iters, c->probe_sink, blocks, threads, c->stream);
+  CU(cudaEventRecord(e1, c->stream));
+  CU(cudaEventSynchronize(e1));
+  c->launches += 2;
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *inst_per_s = (double)blocks * threads * (double)iters * 8.0 / (ms * 1e-3);
+  return check_launch(c, "fp64 probe");
+}
+
+extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used) {
+  int rc = need_metric(c);
+  if (rc) return rc;
+  if (!P_host || nsteps < 0) return fail(c, GRIM_EINVAL, "grim_timestep_host: bad argument");
+  CU(cudaSetDevice(c->d.device));
+  const size_t pbytes = (size_t)c->gv.nvar * c->gv.zg * 8;
+  if (!c->hostP) CU(cudaMalloc((void **)&c->hostP, pbytes));
+  CU(cudaMemcpyAsync(c->hostP, P_host, pbytes, cudaMemcpyHostToDevice, c->stream));
+  for (int s = 0; s < nsteps; s++) {
+    rc = grim_timestep(c, c->hostP, dt, dt_used, nullptr);
+    if (rc) return rc;
+  }
+  CU(cudaMemcpyAsync(P_host, c->hostP, pbytes, cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return GRIM_OK;
+}
+
+extern "C" int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, double *P_host,
+                                           int32_t *iters_host, int32_t *status_host, double *resnorm_host) {
+  if (!c) return GRIM_EINVAL;
+  if (nz < 0 || (nz > 0 && (!U_host || !P_host))) return fail(c, GRIM_EINVAL, "grim_invert_primitives_host: bad argument");
+  if (nz == 0) return GRIM_OK;
+  CU(cudaSetDevice(c->d.device));
+  const size_t N = (size_t)c->gv.nvar;
+  if (c->invbuf_nz < nz) {
+    if (c->invbuf) cudaFree(c->invbuf);
+    c->invbuf = nullptr;
+    CU(cudaMalloc((void **)&c->invbuf, (2 * N + 2) * (size_t)nz * 8));
+    c->invbuf_nz = nz;
+  }
+  double *dU = c->invbuf, *dP = dU + N * nz, *dres = dP + N * nz;
+  int32_t *dit = (int32_t *)(dres + nz), *dst = dit + nz;
+  CU(cudaMemcpyAsync(dU, U_host, N * nz * 8, cudaMemcpyHostToDevice, c->stream));
+  CU(cudaMemcpyAsync(dP, P_host, N * nz * 8, cudaMemcpyHostToDevice, c->stream));
+  int rc = grim_invert_primitives(c, nz, dU, nullptr, dP, dit, dst, dres);
+  if (rc) return rc;
+  CU(cudaMemcpyAsync(P_host, dP, N * nz * 8, cudaMemcpyDeviceToHost, c->stream));
+  if (iters_host) CU(cudaMemcpyAsync(iters_host, dit, (size_t)nz * 4, cudaMemcpyDeviceToHost, c->stream));
+  if (status_host) CU(cudaMemcpyAsync(status_host, dst, (size_t)nz * 4, cudaMemcpyDeviceToHost, c->stream));
+  if (resnorm_host) CU(cudaMemcpyAsync(resnorm_host, dres, (size_t)nz * 8, cudaMemcpyDeviceToHost, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  return GRIM_OK;
+}

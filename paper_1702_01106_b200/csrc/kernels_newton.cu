@@ -1,0 +1,200 @@
+// kernels_newton.cu -- the fused per-zone Newton kernels (steps a4-a7 of the hot path).
+//   newton_stage_kernel : one stage of the time step, one thread per interior zone.  Reads P^k, P_n, P_E, C, G
+//                         once, iterates on chip, writes P^{k'}, ||R||, status, iterations once.
+//   invert_kernel       : standalone primitive recovery on flat arrays, over a compacted list of active zones.
+#include "grim_internal.h"
+#include "problems.cuh"
+
+namespace grim {
+
+static constexpr int NB = 128;  // threads per block; 2 blocks/SM: 2 x 128 x (N*N*8 B) of Jacobian + 255 registers
+
+template <int N, class G>
+__global__ void __launch_bounds__(NB, 2)
+newton_stage_kernel(GridView gv, const double *__restrict__ Pn, const double *__restrict__ PE,
+                    const double *__restrict__ C, const double *__restrict__ Gx, double dt_stage, int max_iters,
+                    double *__restrict__ Piter, double *__restrict__ resnorm, int32_t *__restrict__ status,
+                    int32_t *__restrict__ iters, Counters *cnt) {
+  extern __shared__ double smem[];
+  const long long t = (long long)blockIdx.x * NB + threadIdx.x;
+  int nbt = 0, active_after = 0;
+  if (t < gv.nint) {
+    int i, j, k;
+    zone_coords(gv, t, i, j, k);
+    const long long z = zone_index(gv, i, j, k);
+    int st = status[z];
+    if (!(st & ST_TERMINAL)) {
+      StageProblem<N, G> prob;
+      prob.m = gv.m;
+      if constexpr (G::flat) {
+        prob.tau_ = gv.tau_const;
+      } else {
+        load_geom<0>(gv.geomC, gv.n2d, (long long)j * gv.sz[0] + i, prob.g, prob.tau_);
+      }
+      double P[N];
+      {
+        double Pn_z[N], PE_z[N];
+#pragma unroll
+        for (int v = 0; v < N; v++) {
+          Pn_z[v] = Pn[v * gv.zg + z];
+          PE_z[v] = PE[v * gv.zg + z];
+          P[v] = Piter[v * gv.zg + z];
+          prob.C[v] = C[v * gv.zg + z];
+        }
+        if constexpr (N == 10) {
+          prob.Xq = Gx[0 * gv.zg + z];
+          prob.Xd = Gx[1 * gv.zg + z];
+          prob.divx = Gx[2 * gv.zg + z];
+        }
+        prob.setup(Pn_z, PE_z, dt_stage);
+      }
+      const double tol = gv.sp.atol + gv.sp.rtol * prob.scale;
+      int it = iters[z];
+      JacView<N, NB> jac{smem + threadIdx.x};
+      double rn = newton_zone<N, NB>(prob, gv.sp, tol, P, it, st, max_iters, jac, nbt);
+#pragma unroll
+      for (int v = 0; v < N; v++) Piter[v * gv.zg + z] = P[v];
+      resnorm[z] = rn;
+      status[z] = st;
+      iters[z] = it;
+      active_after = (st & ST_TERMINAL) ? 0 : 1;
+    }
+  }
+  // warp-aggregated counters
+  unsigned long long a = __reduce_add_sync(0xffffffffu, (unsigned)active_after);
+  unsigned long long b = __reduce_add_sync(0xffffffffu, (unsigned)nbt);
+  if ((threadIdx.x & 31) == 0) {
+    if (a) atomicAdd(&cnt->n_active, a);
+    if (b) atomicAdd(&cnt->backtracks, b);
+  }
+}
+
+template <int N, class G>
+static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *Gx,
+                          double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
+                          int32_t *iters, Counters *cnt, cudaStream_t s) {
+  const size_t smem = (size_t)N * N * NB * sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(newton_stage_kernel<N, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_set = true;
+  }
+  const long long blocks = (gv.nint + NB - 1) / NB;
+  newton_stage_kernel<N, G><<<(unsigned)blocks, NB, smem, s>>>(gv, Pn, PE, C, Gx, dt_stage, max_iters, Piter,
+                                                               resnorm, status, iters, cnt);
+  return 1;
+}
+
+int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *G,
+                        double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
+                        int32_t *iters, Counters *cnt, cudaStream_t s) {
+  const bool flat = (gv.metric == 0);
+  if (gv.nvar == 10) {
+    return flat ? launch_stage_t<10, GeomFlat>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
+                : launch_stage_t<10, GeomGen>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
+  }
+  return flat ? launch_stage_t<8, GeomFlat>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
+              : launch_stage_t<8, GeomGen>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Standalone inversion.  `first` != 0: thread t handles zone t of all nz zones, iters/status start at zero.
+// Otherwise thread t handles zone list[t], t < nlist.  Zones left without a terminal status are appended to
+// next_list (order is not deterministic; the per-zone results are).
+// ---------------------------------------------------------------------------------------------------------
+template <int N>
+__global__ void __launch_bounds__(NB, 2)
+invert_kernel(GridView gv, long long nz, long long nlist, const long long *__restrict__ list,
+              const double *__restrict__ Ustar, double *__restrict__ Pio, int32_t *__restrict__ iters,
+              int32_t *__restrict__ status, double *__restrict__ resnorm, int max_iters, int first,
+              long long *__restrict__ next_list, Counters *cnt) {
+  extern __shared__ double smem[];
+  const long long t = (long long)blockIdx.x * NB + threadIdx.x;
+  int nbt = 0, active_after = 0;
+  long long z = -1;
+  if (t < nlist) {
+    z = first ? t : list[t];
+    InvertProblem<N> prob;
+    prob.m = gv.m;
+    prob.tau_ = gv.tau_const;
+    double P[N];
+#pragma unroll
+    for (int v = 0; v < N; v++) {
+      prob.Ustar[v] = Ustar[v * nz + z];
+      P[v] = Pio[v * nz + z];
+    }
+    prob.setup();
+    int it = first ? 0 : iters[z];
+    int st = first ? 0 : status[z];
+    JacView<N, NB> jac{smem + threadIdx.x};
+    double rn = newton_zone<N, NB>(prob, gv.sp, gv.sp.rtol, P, it, st, max_iters, jac, nbt);
+#pragma unroll
+    for (int v = 0; v < N; v++) Pio[v * nz + z] = P[v];
+    resnorm[z] = rn;
+    status[z] = st;
+    iters[z] = it;
+    active_after = (st & ST_TERMINAL) ? 0 : 1;
+  }
+  // warp-aggregated append to the next active list
+  const unsigned ballot = __ballot_sync(0xffffffffu, active_after);
+  const int lane = threadIdx.x & 31;
+  unsigned long long base = 0;
+  if (lane == 0 && ballot) base = atomicAdd(&cnt->list_count, (unsigned long long)__popc(ballot));
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (active_after) next_list[base + __popc(ballot & ((1u << lane) - 1u))] = z;
+  unsigned long long b = __reduce_add_sync(0xffffffffu, (unsigned)nbt);
+  if (lane == 0 && b) atomicAdd(&cnt->backtracks, b);
+}
+
+template <int N>
+static int launch_invert_t(const GridView &gv, long long nz, long long nlist, const long long *list,
+                           const double *Ustar, double *P, int32_t *iters, int32_t *status, double *resnorm,
+                           int max_iters, int first, long long *next_list, Counters *cnt, cudaStream_t s) {
+  const size_t smem = (size_t)N * N * NB * sizeof(double);
+  static bool attr_set = false;
+  if (!attr_set) {
+    cudaFuncSetAttribute(invert_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    attr_set = true;
+  }
+  const long long blocks = (nlist + NB - 1) / NB;
+  if (blocks == 0) return 0;
+  invert_kernel<N><<<(unsigned)blocks, NB, smem, s>>>(gv, nz, nlist, list, Ustar, P, iters, status, resnorm,
+                                                      max_iters, first, next_list, cnt);
+  return 1;
+}
+
+int launch_invert(const GridView &gv, long long nz, long long nlist, const long long *list, const double *Ustar,
+                  double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters, int first,
+                  long long *next_list, Counters *cnt, cudaStream_t s) {
+  if (gv.nvar == 10)
+    return launch_invert_t<10>(gv, nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list, cnt, s);
+  return launch_invert_t<8>(gv, nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list, cnt, s);
+}
+
+// U(P) on flat arrays, Minkowski (workload construction on the device)
+template <int N>
+__global__ void prim_to_conserved_kernel(GridView gv, long long nz, const double *__restrict__ Pin,
+                                         double *__restrict__ Uout) {
+  const long long z = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (z >= nz) return;
+  double P[N], U[N];
+#pragma unroll
+  for (int v = 0; v < N; v++) P[v] = Pin[v * nz + z];
+  Pieces pc;
+  GeomFlat g;
+  full_state<N>(gv.m, g, gv.tau_const, P, pc.th, pc.v, pc.b, pc.h);
+  flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
+#pragma unroll
+  for (int v = 0; v < N; v++) Uout[v * nz + z] = U[v];
+}
+
+int launch_prim_to_conserved(const GridView &gv, long long nz, const double *P, double *U, cudaStream_t s) {
+  const int tb = 256;
+  const long long blocks = (nz + tb - 1) / tb;
+  if (blocks == 0) return 0;
+  if (gv.nvar == 10) prim_to_conserved_kernel<10><<<(unsigned)blocks, tb, 0, s>>>(gv, nz, P, U);
+  else prim_to_conserved_kernel<8><<<(unsigned)blocks, tb, 0, s>>>(gv, nz, P, U);
+  return 1;
+}
+
+}  // namespace grim

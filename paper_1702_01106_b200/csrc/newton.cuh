@@ -1,0 +1,245 @@
+// newton.cuh -- the per-zone Newton-Raphson iteration of grim (eqs 20-25), one thread per
+// zone, the whole iteration on chip:
+//   * residual pieces cached in registers and reused by the finite-difference columns they do not depend on
+//     (eqs 22-23; G-4, C-16, C-17),
+//   * the N x N Jacobian in shared memory, one column of 8-byte words per thread (bank-conflict free for any
+//     run-time row index), factorised by a left-looking LU with partial pivoting whose row exchanges are
+//     exchanges of row *pointers* held in registers (eq 21; L434 "LAPACK" -> dgetf2/dgesv semantics: pivot =
+//     first row of maximal |a_ik|, multipliers formed with the reciprocal of the pivot; C-19),
+//   * quadratic backtracking line search (L218-235, eqs 24-25; G-2, C-14).
+// The left-looking order applies to every matrix element the same updates in the same order (k ascending) as
+// the textbook right-looking elimination, so the factors are identical; it reads each multiplier column from
+// shared memory once per later column and writes each element once.
+#pragma once
+
+#include "physics.cuh"
+
+namespace grim {
+
+struct SolverParams {
+  double fd_eps, eps_bt, atol, rtol;
+  int kmax, lsmax;
+};
+
+enum {
+  ST_CONVERGED = 1, ST_KMAX = 2, ST_LS_EXHAUSTED = 4, ST_SINGULAR = 8, ST_NONFINITE = 16,
+  ST_TERMINAL = ST_CONVERGED | ST_KMAX | ST_SINGULAR | ST_NONFINITE
+};
+
+struct Pieces {
+  Thermo th;
+  Vel v;
+  Mag b;
+  BHat h;
+};
+
+template <int N>
+__device__ __forceinline__ double norm2sq(const double (&R)[N]) {
+  double s = R[0] * R[0];
+#pragma unroll
+  for (int v = 1; v < N; v++) s = s + R[v] * R[v];
+  return s;
+}
+
+// Residual at P with every piece recomputed; the pieces are returned for reuse.
+template <int N, class Prob>
+__device__ __forceinline__ void eval_full(const Prob &prob, const double (&P)[N], Pieces &pc, double (&R)[N]) {
+  full_state<N>(prob.model(), prob.geom(), prob.tau(), P, pc.th, pc.v, pc.b, pc.h);
+  prob.assemble(P, pc, R);
+}
+
+// Residual at P with component J replaced by pj (eq 23): only the pieces that depend on component J are
+// recomputed; the others are those of the unperturbed state.
+template <int J, int N, class Prob>
+__device__ __forceinline__ void eval_column(const Prob &prob, const double (&P)[N], double pj, const Pieces &base,
+                                            double (&R)[N]) {
+  double Pe[N];
+#pragma unroll
+  for (int v = 0; v < N; v++) Pe[v] = P[v];
+  Pe[J] = pj;
+  Pieces pc = base;
+  if constexpr (J == RHO || J == UU) {
+    thermo_state<N>(prob.model(), prob.tau(), Pe[RHO], Pe[UU], pc.th);
+  } else if constexpr (J >= U1 && J <= U3) {
+    vel_state(prob.geom(), Pe[U1], Pe[U2], Pe[U3], pc.v);
+    mag_state(prob.geom(), pc.v, Pe[B1], Pe[B2], Pe[B3], pc.b);
+    if constexpr (N == 10) bhat_state(pc.b, pc.h);
+  } else if constexpr (J >= B1 && J <= B3) {
+    mag_state(prob.geom(), pc.v, Pe[B1], Pe[B2], Pe[B3], pc.b);
+    if constexpr (N == 10) bhat_state(pc.b, pc.h);
+  }
+  prob.assemble(Pe, pc, R);
+}
+
+// Shared-memory Jacobian of one thread: element (row r, column c) at sJ[(r*N + c)*BLOCK], sJ already offset by
+// the thread index.
+template <int N, int BLOCK>
+struct JacView {
+  double *base;
+  __device__ __forceinline__ double &at(int rowoff, int c) const { return base[rowoff + c * BLOCK]; }
+  static __device__ __forceinline__ constexpr int row(int r) { return r * N * BLOCK; }
+};
+
+// One finite-difference column (eqs 22-23): J[:,j] = (R(P_eps,j) - R0) / (P_eps,j - P_j)
+template <int J, int N, int BLOCK, class Prob>
+__device__ __forceinline__ void fd_column(const Prob &prob, const SolverParams &sp, const double (&P)[N],
+                                          const Pieces &base, const double (&R0)[N], const JacView<N, BLOCK> &jac,
+                                          bool &singular) {
+  double pj = (fabs(P[J]) < 5.0 * sp.fd_eps) ? sp.fd_eps : (1.0 + sp.fd_eps) * P[J];
+  double h = pj - P[J];
+  if (h == 0.0) singular = true;
+  double ih = 1.0 / h;
+  double Rt[N];
+  eval_column<J, N>(prob, P, pj, base, Rt);
+#pragma unroll
+  for (int i = 0; i < N; i++) jac.at(JacView<N, BLOCK>::row(i), J) = (Rt[i] - R0[i]) * ih;
+}
+
+template <int J, int N, int BLOCK, class Prob>
+struct FdColumns {
+  static __device__ __forceinline__ void run(const Prob &prob, const SolverParams &sp, const double (&P)[N],
+                                             const Pieces &base, const double (&R0)[N],
+                                             const JacView<N, BLOCK> &jac, bool &singular) {
+    fd_column<J, N, BLOCK>(prob, sp, P, base, R0, jac, singular);
+    FdColumns<J + 1, N, BLOCK, Prob>::run(prob, sp, P, base, R0, jac, singular);
+  }
+};
+template <int N, int BLOCK, class Prob>
+struct FdColumns<N, N, BLOCK, Prob> {
+  static __device__ __forceinline__ void run(const Prob &, const SolverParams &, const double (&)[N], const Pieces &,
+                                             const double (&)[N], const JacView<N, BLOCK> &, bool &) {}
+};
+
+// Solves J x = b (b in, x out) for the Jacobian held in shared memory.  Returns false if a pivot is zero or
+// non-finite (C-19).
+template <int N, int BLOCK>
+__device__ __forceinline__ bool lu_solve(const JacView<N, BLOCK> &jac, double (&b)[N]) {
+  int rowoff[N];
+  double rinv[N];
+#pragma unroll
+  for (int i = 0; i < N; i++) rowoff[i] = JacView<N, BLOCK>::row(i);
+  bool ok = true;
+#pragma unroll
+  for (int j = 0; j < N; j++) {
+    double x[N];
+#pragma unroll
+    for (int i = 0; i < N; i++) x[i] = jac.at(rowoff[i], j);
+    // updates of the earlier pivots, k ascending; the last column carries the right-hand side along
+#pragma unroll
+    for (int k = 0; k < j; k++) {
+#pragma unroll
+      for (int i = k + 1; i < N; i++) {
+        double l = jac.at(rowoff[i], k);
+        x[i] = x[i] - l * x[k];
+        if (j == N - 1) b[i] = b[i] - l * b[k];
+      }
+    }
+    // pivot: first row of maximal |x_i|, i >= j
+    int p = j;
+    double amax = fabs(x[j]);
+#pragma unroll
+    for (int i = j + 1; i < N; i++) {
+      double v = fabs(x[i]);
+      if (v > amax) {
+        amax = v;
+        p = i;
+      }
+    }
+    if (!(amax > 0.0) || !isfinite(amax)) ok = false;
+#pragma unroll
+    for (int i = j + 1; i < N; i++) {
+      if (p == i) {
+        double t = x[j]; x[j] = x[i]; x[i] = t;
+        t = b[j]; b[j] = b[i]; b[i] = t;
+        int o = rowoff[j]; rowoff[j] = rowoff[i]; rowoff[i] = o;
+      }
+    }
+    double r = 1.0 / x[j];
+    rinv[j] = r;
+#pragma unroll
+    for (int i = j + 1; i < N; i++) x[i] = x[i] * r;
+#pragma unroll
+    for (int i = 0; i < N; i++) jac.at(rowoff[i], j) = x[i];
+  }
+  // back substitution with U
+#pragma unroll
+  for (int i = N - 1; i >= 0; i--) {
+    double s = b[i];
+#pragma unroll
+    for (int j = i + 1; j < N; j++) s = s - jac.at(rowoff[i], j) * b[j];
+    b[i] = s * rinv[i];
+  }
+  return ok;
+}
+
+// eq 25 (L230): minimiser of the quadratic through f(0), f'(0) = -2 f(0), f(lam)
+__device__ __forceinline__ double linesearch_lambda(double f0, double flam, double lam) {
+  return f0 / (flam + (2.0 * lam - 1.0) * f0) * lam * lam;
+}
+
+// Runs at most max_iters further Newton iterations (<= 0: until terminal) of one zone.  P, iters, status carry
+// the zone's state between calls.  Returns ||R(P)||_2 of the final state.
+template <int N, int BLOCK, class Prob>
+__device__ __forceinline__ double newton_zone(const Prob &prob, const SolverParams &sp, double tol, double (&P)[N],
+                                              int &iters, int &status, int max_iters,
+                                              const JacView<N, BLOCK> &jac, int &backtracks) {
+  double R0[N];
+  Pieces pc;
+  int k = iters, st = status, done = 0;
+  eval_full<N>(prob, P, pc, R0);
+  double f0 = norm2sq<N>(R0);
+  if (!isfinite(f0)) {
+    status = st | ST_NONFINITE;
+    return sqrt(f0);
+  }
+  while (!(sqrt(f0) < tol) && k < sp.kmax && (max_iters <= 0 || done < max_iters)) {
+    bool singular = false;
+    FdColumns<0, N, BLOCK, Prob>::run(prob, sp, P, pc, R0, jac, singular);
+    double dP[N];
+#pragma unroll
+    for (int v = 0; v < N; v++) dP[v] = -R0[v];
+    bool ok = lu_solve<N, BLOCK>(jac, dP);
+    if (singular || !ok) {
+      st |= ST_SINGULAR;
+      break;
+    }
+    double lam = 1.0, ft = f0;
+    bool accepted = false;
+    double Pt[N], Rt[N];
+    for (int ls = 0; ls <= sp.lsmax; ls++) {
+#pragma unroll
+      for (int v = 0; v < N; v++) Pt[v] = P[v] + lam * dP[v];
+      eval_full<N>(prob, Pt, pc, Rt);
+      ft = norm2sq<N>(Rt);
+      if (sqrt(ft) < sqrt(f0) * (1.0 - sp.eps_bt * lam)) {
+        accepted = true;
+        break;
+      }
+      if (ls == sp.lsmax) break;
+      backtracks++;
+      lam = isfinite(ft) ? linesearch_lambda(f0, ft, lam) : 0.5 * lam;
+    }
+    if (!accepted) st |= ST_LS_EXHAUSTED;
+#pragma unroll
+    for (int v = 0; v < N; v++) {
+      P[v] = Pt[v];
+      R0[v] = Rt[v];
+    }
+    f0 = ft;
+    k++;
+    done++;
+    if (!isfinite(f0)) {
+      st |= ST_NONFINITE;
+      break;
+    }
+  }
+  if (!(st & (ST_SINGULAR | ST_NONFINITE))) {
+    if (sqrt(f0) < tol) st |= ST_CONVERGED;
+    else if (k >= sp.kmax) st |= ST_KMAX;
+  }
+  iters = k;
+  status = st;
+  return sqrt(f0);
+}
+
+}  // namespace grim

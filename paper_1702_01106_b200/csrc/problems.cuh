@@ -1,0 +1,120 @@
+// problems.cuh -- the two residual functions the Newton iteration is applied to.
+//   StageProblem : residual of one stage of the semi-implicit time step (eq 19 L185-188 half step, eq 13
+//                  L127-130 full step; eqs 15-16; EMHD rows eqs 39-40; readings C-3, C-4)
+//   InvertProblem: standalone primitive recovery R(P) = (U(P) - U*)/||U*||_2 (O-10; BASELINE config 2)
+#pragma once
+
+#include "newton.cuh"
+
+namespace grim {
+
+template <int N, class G>
+struct StageProblem {
+  ModelParams m;
+  G g;
+  double tau_, idt, itau;
+  double C[N];
+  double scale;  // ||U(P_n)||_2 / dt' (C-2)
+  // EMHD only.  P_n-derived:
+  double Thn, ucovn[4], utn, qtn, dtn;
+  // P_E-derived coefficients, frozen during the iteration (O-8), and the spatial-gradient terms of the stage:
+  double bh[4], ThE, utE, nrhochi, rhonu3, fqE, fdE, hqtE, hdtE;
+  double Xq, Xd, divx;
+
+  __device__ __forceinline__ const ModelParams &model() const { return m; }
+  __device__ __forceinline__ const G &geom() const { return g; }
+  __device__ __forceinline__ double tau() const { return tau_; }
+
+  // Everything that depends only on P_n and P_E (L438)
+  __device__ __forceinline__ void setup(const double (&Pn)[N], const double (&PE)[N], double dt_stage) {
+    idt = 1.0 / dt_stage;
+    itau = 1.0 / tau_;
+    Pieces pn;
+    full_state<N>(m, g, tau_, Pn, pn.th, pn.v, pn.b, pn.h);
+    double Un[N];
+    flux_vector<N>(g, 0, Pn, pn.th, pn.v, pn.b, pn.h, Un);
+    scale = sqrt(norm2sq<N>(Un)) * idt;
+    if constexpr (N == 10) {
+      Thn = pn.th.Th;
+#pragma unroll
+      for (int i = 0; i < 4; i++) ucovn[i] = pn.v.ucov[i];
+      utn = pn.v.ucon[0];
+      qtn = Pn[QQ] * pn.th.fq;
+      dtn = Pn[DPP] * pn.th.fdp;
+      Pieces pe;
+      full_state<N>(m, g, tau_, PE, pe.th, pe.v, pe.b, pe.h);
+#pragma unroll
+      for (int i = 0; i < 4; i++) bh[i] = pe.h.con[i];
+      ThE = pe.th.Th;
+      utE = pe.v.ucon[0];
+      double cs2 = sound_speed2(m, PE[RHO], PE[UU]);
+      double chi = m.phi * cs2 * tau_, nu = m.psi * cs2 * tau_;
+      nrhochi = -(PE[RHO] * chi);
+      rhonu3 = 3.0 * PE[RHO] * nu;
+      fqE = pe.th.fq;
+      fdE = pe.th.fdp;
+      hqtE = 0.5 * (PE[QQ] * fqE);
+      hdtE = 0.5 * (PE[DPP] * fdE);
+    }
+  }
+
+  __device__ __forceinline__ void assemble(const double (&P)[N], const Pieces &pc, double (&R)[N]) const {
+    double U[N];
+    flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
+#pragma unroll
+    for (int v = 0; v < N; v++) R[v] = U[v] * idt + C[v];
+    if constexpr (N == 10) {
+      // time derivatives of derived quantities between the unknown state and P_n (C-3)
+      double dtTheta = (pc.th.Th - Thn) * idt;
+      double dtucov[4];
+#pragma unroll
+      for (int i = 0; i < 4; i++) dtucov[i] = (pc.v.ucov[i] - ucovn[i]) * idt;
+      double dtut = (pc.v.ucon[0] - utn) * idt;
+      double bdu = bh[0] * dtucov[0];
+      bdu = bdu + bh[1] * dtucov[1];
+      bdu = bdu + bh[2] * dtucov[2];
+      bdu = bdu + bh[3] * dtucov[3];
+      double Tq = bh[0] * dtTheta + ThE * (utE * bdu);
+      double Td = bh[0] * bdu;
+      double divu = dtut + divx;
+      double q0 = nrhochi * (Tq + Xq);                              // eq 37
+      double dP0 = rhonu3 * ((Td + Xd) - (1.0 / 3.0) * divu);        // eq 38 (G-5)
+      double qt = P[QQ] * pc.th.fq, dpt = P[DPP] * pc.th.fdp;
+      double Sq = -(0.5 * (qt + qtn) - fqE * q0) * itau + hqtE * divu;    // eq 39, eqs 15-16
+      double Sd = -(0.5 * (dpt + dtn) - fdE * dP0) * itau + hdtE * divu;  // eq 40
+      if constexpr (G::flat) {
+        R[QQ] = R[QQ] - Sq;
+        R[DPP] = R[DPP] - Sd;
+      } else {
+        R[QQ] = R[QQ] - g.sqrtmg() * Sq;
+        R[DPP] = R[DPP] - g.sqrtmg() * Sd;
+      }
+    }
+  }
+};
+
+template <int N>
+struct InvertProblem {
+  ModelParams m;
+  GeomFlat g;
+  double tau_;
+  double Ustar[N];
+  double iscale;
+
+  __device__ __forceinline__ const ModelParams &model() const { return m; }
+  __device__ __forceinline__ const GeomFlat &geom() const { return g; }
+  __device__ __forceinline__ double tau() const { return tau_; }
+
+  __device__ __forceinline__ void setup() {
+    double s2 = norm2sq<N>(Ustar);
+    iscale = 1.0 / sqrt(s2);
+  }
+  __device__ __forceinline__ void assemble(const double (&P)[N], const Pieces &pc, double (&R)[N]) const {
+    double U[N];
+    flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
+#pragma unroll
+    for (int v = 0; v < N; v++) R[v] = (U[v] - Ustar[v]) * iscale;
+  }
+};
+
+}  // namespace grim

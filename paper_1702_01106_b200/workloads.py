@@ -1,0 +1,93 @@
+"""Seeded synthetic inputs shaped like the paper's workloads (BASELINE.json configs; recipes in DESIGN.md).
+
+numpy only.  This module holds none of the method's arithmetic: it produces primitive-variable arrays (initial
+data), guesses and grid descriptions, and serves both the oracle (tests, cpu_baseline) and the CUDA library
+(tests, bench.py).  The linear-mode eigenvectors come from data/linear_modes.json, written by
+oracle/write_mode_tables.py.  No public dataset is involved: the paper's tests are analytic initial data.
+"""
+import json
+import os
+
+import numpy as np
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+_modes = None
+
+
+def mode_tables():
+    global _modes
+    if _modes is None:
+        with open(os.path.join(HERE, "data", "linear_modes.json")) as f:
+            _modes = json.load(f)
+    return _modes
+
+
+def padded_centres(n, ngd, xstart, xend):
+    """Zone-centre coordinates X^1, X^2, X^3 of the padded grid, each of shape [s3, s2, s1]."""
+    ax = []
+    for a in range(3):
+        dx = (xend[a] - xstart[a]) / n[a]
+        ax.append(xstart[a] + (np.arange(n[a] + 2 * ngd[a]) - ngd[a] + 0.5) * dx)
+    X3, X2, X1 = np.meshgrid(ax[2], ax[1], ax[0], indexing="ij")
+    return X1, X2, X3
+
+
+def linear_mode_state(P0, modes, amp, X1, X2, X3):
+    """P = P0 + amp * sum_m Re[dP_m exp(i (k_m . x + phase_m))]."""
+    P0 = np.asarray(P0, dtype=np.float64)
+    P = np.repeat(P0[:, None], X1.size, axis=1).reshape((len(P0),) + X1.shape).copy()
+    for md in modes:
+        k = md["k"]
+        dP = np.asarray(md["dP_re"]) + 1j * np.asarray(md["dP_im"])
+        ph = np.exp(1j * (k[0] * X1 + k[1] * X2 + k[2] * X3 + md.get("phase", 0.0)))
+        P += amp * (dP[:, None, None, None] * ph[None]).real
+    return P
+
+
+def config1(n=64, amp=1e-4):
+    """Ideal MHD, 2-D Minkowski, n x n periodic on [0,1]^2, fast mode k = (2 pi, 2 pi), minmod, LLF, cfl 0.5."""
+    t = mode_tables()["config1"]
+    grid = dict(n1=n, n2=n, n3=1, ng=3, dim=2, xstart=(0.0, 0.0, 0.0), xend=(1.0, 1.0, 1.0), nvar=8, recon=0,
+                limiter_theta=1.0, gam=t["gamma"], rtol=1e-14, kmax=8, lsmax=5, cfl=0.5)
+    X = padded_centres((n, n, 1), (3, 3, 0), grid["xstart"], grid["xend"])
+    return grid, linear_mode_state(t["P0"], t["modes"], amp, *X)
+
+
+def config3(n=128, amp=1e-4, dim=3, recon=1):
+    """EMHD, 3-D Minkowski, n^3 periodic on [0,1]^3, four seeded random-phase linear modes, MP5, LLF, cfl 0.5.
+    The headline run is the same generator at n = 256."""
+    t = mode_tables()["config3"]
+    nn = (n, n, n if dim == 3 else 1)
+    grid = dict(n1=nn[0], n2=nn[1], n3=nn[2], ng=3, dim=dim, xstart=(0.0, 0.0, 0.0), xend=(1.0, 1.0, 1.0), nvar=10,
+                recon=recon, limiter_theta=1.0, gam=t["gamma"], phi=t["phi"], psi=t["psi"], tau=t["tau"],
+                rtol=1e-14, kmax=8, lsmax=5, cfl=0.5)
+    ngd = (3, 3, 3 if dim == 3 else 0)
+    X = padded_centres(nn, ngd, grid["xstart"], grid["xend"])
+    return grid, linear_mode_state(t["P0"], t["modes"], amp, *X)
+
+
+def config2(nz, seed=1702, nvar=8):
+    """Standalone primitive recovery (BASELINE config 2): rho, u log-uniform in [1e-4, 1e2]; Lorentz factor
+    uniform in [1, 10], isotropic direction; |B|^2/rho log-uniform in [1e-3, 1e2], isotropic; guess = P (1 + 0.1 xi),
+    xi ~ U[-1,1] per component (C-20).  For nvar = 10, q and dP are small seeded fractions of rho Theta^{3/2} and
+    of the pressure.  Returns (P_true, P_guess), each [nvar, nz]."""
+    rng = np.random.Generator(np.random.PCG64(seed))
+    P = np.zeros((nvar, nz))
+    P[0] = np.exp(rng.uniform(np.log(1e-4), np.log(1e2), nz))
+    P[1] = np.exp(rng.uniform(np.log(1e-4), np.log(1e2), nz))
+    W = rng.uniform(1.0, 10.0, nz)
+    d = rng.standard_normal((3, nz))
+    d /= np.linalg.norm(d, axis=0, keepdims=True)
+    P[2:5] = np.sqrt(W * W - 1.0) * d
+    Bsq = P[0] * np.exp(rng.uniform(np.log(1e-3), np.log(1e2), nz))
+    d = rng.standard_normal((3, nz))
+    d /= np.linalg.norm(d, axis=0, keepdims=True)
+    P[5:8] = np.sqrt(Bsq) * d
+    xi = rng.uniform(-1.0, 1.0, (nvar, nz))
+    if nvar == 10:
+        pg = P[1] / 3.0
+        P[8] = 0.1 * rng.uniform(-1.0, 1.0, nz) * P[0] * (pg / P[0]) ** 1.5
+        P[9] = 0.1 * rng.uniform(-1.0, 1.0, nz) * pg
+    guess = P * (1.0 + 0.1 * xi)
+    return P, guess

@@ -1,0 +1,86 @@
+"""Host-side checks of the C-ABI library that need no GPU: it builds, loads, exports every symbol include/grim.h
+declares, validates arguments, and fails loudly (no CPU fallback) without a device."""
+import ctypes as C
+import os
+import re
+
+import pytest
+
+import paper_1702_01106_b200 as gb
+from paper_1702_01106_b200 import build as gbuild
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def L():
+    gbuild.build()
+    return gb.lib()
+
+
+def test_exports_every_declared_symbol(L):
+    hdr = open(os.path.join(ROOT, "include", "grim.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = sorted(set(re.findall(r"\b(grim_[a-z0-9_]+)\s*\(", hdr)))
+    assert len(declared) >= 12
+    for name in declared:
+        assert hasattr(L, name), name
+    assert declared == gb.exported_symbols()
+    for six in ("grim_init_grid", "grim_set_metric", "grim_compute_fluxes", "grim_newton_step",
+                "grim_invert_primitives", "grim_timestep"):
+        assert six in declared
+
+
+def test_version_and_struct_layout(L):
+    assert L.grim_version() == 100
+    # the structs the binding marshals must have the layout a C compiler gives include/grim.h
+    import subprocess
+    import tempfile
+    with tempfile.TemporaryDirectory() as td:
+        src = os.path.join(td, "sz.c")
+        open(src, "w").write('#include <stdio.h>\n#include <stddef.h>\n#include "grim.h"\nint main(void){printf("%zu %zu %zu %zu\\n",'
+                             'sizeof(grim_grid_desc), sizeof(grim_step_stats), offsetof(grim_grid_desc, cfl),'
+                             'offsetof(grim_grid_desc, stream));return 0;}\n')
+        exe = os.path.join(td, "sz")
+        subprocess.check_call(["gcc", "-I", os.path.join(ROOT, "include"), src, "-o", exe])
+        sizes = [int(x) for x in subprocess.check_output([exe]).split()]
+    assert sizes == [C.sizeof(gb.GridDesc), C.sizeof(gb.StepStats), gb.GridDesc.cfl.offset, gb.GridDesc.stream.offset]
+
+
+def test_init_validates_before_touching_the_device(L):
+    d = gb.GridDesc()
+    h = C.c_void_p()
+    d.n1, d.n2, d.n3, d.ng, d.dim, d.model = 8, 8, 1, 3, 4, 10
+    assert L.grim_init_grid(C.byref(h), C.byref(d)) == -1          # GRIM_EINVAL: dim
+    assert b"dim" in L.grim_last_error(None)
+    d.dim, d.model = 2, 9
+    assert L.grim_init_grid(C.byref(h), C.byref(d)) == -1          # model
+    d.model, d.recon, d.ng = 10, 1, 2
+    assert L.grim_init_grid(C.byref(h), C.byref(d)) == -1          # MP5 needs ng >= 3
+    assert h.value is None
+    assert L.grim_init_grid(None, None) == -1
+
+
+def test_no_cpu_fallback(L):
+    """Without a usable sm_100 device the library refuses to create a context (GRIM_ECUDA), it never computes on
+    the host.  (On the GPU box this test checks that a context can be created instead.)"""
+    import torch
+    if torch.cuda.is_available():
+        g = gb.Grid(8, 8, 1, ng=3, dim=2)
+        assert g.h
+        g.close()
+    else:
+        with pytest.raises(gb.GrimError, match="no CUDA device|CPU fallback|sm_100"):
+            gb.Grid(8, 8, 1, ng=3, dim=2)
+
+
+def test_product_does_not_import_oracle():
+    """The product path may not route through the oracle: no file of the package mentions it in code."""
+    pkg = os.path.join(ROOT, "paper_1702_01106_b200")
+    for dp, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                src = open(os.path.join(dp, f)).read()
+                code = re.sub(r'""".*?"""', "", src, flags=re.S)
+                code = re.sub(r"//.*|#.*", "", code)
+                assert "import oracle" not in code and "grim_oracle" not in code and "libgrim_oracle" not in code, f
