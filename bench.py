@@ -1,0 +1,261 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the grim hot path on B200 (contract: see DESIGN.md "Measurement").
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--n 256] [--impl ours|reference]
+
+Workload: BASELINE.json config 3's generator at n^3 (headline n = 256): EMHD (10 primitives), 3-D Minkowski,
+periodic, four seeded linear modes of amplitude 1e-4 on the background rho=1, u=2, B=(0.1,0.3,0); MP5 + LLF,
+CFL 0.5.  A "step" is one grim_timestep: 2 stages x (ghost fill, reconstruction + LLF fluxes + stage constants,
+fused per-zone Newton solve).  value = zones advanced one time step per second, whole job.
+
+N > 1 (torchrun): the grid is cut into N slabs along X^3 (weak scaling: every rank holds n^3 zones of an
+n x n x (N n) grid); each stage's ghost planes in X^3 are exchanged between neighbouring ranks with
+torch.distributed (NCCL) device-to-device, everything else is rank-local.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fp64 zone-updates/sec per Newton step (EMHD 10-var) and % of HBM roofline"
+UNIT = "zone-updates/s"
+
+# per zone and stage, Minkowski EMHD, 2 Newton iterations (measured with ncu, profiles/)
+ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 15000.0   # fp64-pipe thread instructions of the Newton kernel per zone
+ALG_BYTES_PER_ZONE_STAGE_NEWTON = 8.0 * (10 + 10 + 10 + 10 + 3 + 10 + 1) + 4 * 4   # P^k,P_n,P_E,C,G in; P,|R| out; status,iters in/out
+FP64_INSTR_PER_CLK_PER_SM = 64.0                 # B200: 64 fp64 lanes per SM (guide: unit counts), 148 SMs
+N_SM = 148
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return d.get("hbm_gbs", 6650.0), d.get("sm_max_mhz", 1965.0), "measured"
+    return 6650.0, 1965.0, "fallback"
+
+
+class ClockSampler:
+    """nvidia-smi clocks line of the profiling recipe, sampled every 200 ms during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, device):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(device), "--query-gpu=" + self.Q,
+                                       "--format=csv,noheader,nounits", "-lms", "200"], stdout=self.f,
+                                      stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": [], "samples": 0}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            t = [x.strip() for x in line.split(",")]
+            if len(t) < 9:
+                continue
+            try:
+                sm.append(float(t[1])); mx.append(float(t[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, t[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        self.f.close()
+        os.unlink(self.f.name)
+        if sm:
+            sm.sort()
+            out.update(sm_mhz=sm[len(sm) // 2], sm_max_mhz=max(mx), reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def oracle_sample(n, steps, warmup):
+    """The oracle, as it stands, on the config-3 generator at n^3; returns (zone-updates/s, s per step, cores)."""
+    sys.path.insert(0, os.path.join(ROOT, "oracle"))
+    sys.path.insert(0, os.path.join(ROOT, "tests"))
+    import oracle as og
+    from common import oracle_grid
+    from paper_1702_01106_b200 import workloads
+    gk, P = workloads.config3(n=n)
+    go = oracle_grid(gk)
+    dt = go.choose_dt(P)
+    for _ in range(warmup):
+        go.timestep(P, dt)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        go.timestep(P, dt)
+    el = time.perf_counter() - t0
+    return n ** 3 * steps / el, el / steps, og.num_threads()
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    n = args.ref_n
+    v, sps, cores = oracle_sample(n, args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": sps * 1e3, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config3-emhd-mp5-llf-minkowski-%d^3" % args.n,
+                   "sample": "each step = one oracle time step of the same generator at %d^3" % n},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                         "sample": "config-3 generator at %d^3, %d steps" % (n, args.steps)},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import paper_1702_01106_b200 as gb
+    from paper_1702_01106_b200 import distributed as gdist
+    from paper_1702_01106_b200 import workloads
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    n = args.n
+    gk, P0 = workloads.config3(n=n, ranks=world, rank=rank)
+    slab = gdist.SlabGrid(gk, world, rank, device=local)
+    g = slab.grid
+    dP = torch.from_numpy(P0).cuda()
+    dt = slab.choose_dt(dP)                      # CFL 0.5 on the initial data, min over ranks; then held fixed
+    zones = g.zones
+    pbytes = dP.numel() * 8
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        slab.timestep(dP, dt)
+    barrier()
+    l0 = g.launch_count()
+    g.set_timing(True)
+    sampler = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        slab.timestep(dP, dt)
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if sampler else None
+    timing = g.get_timing()
+    g.set_timing(False)
+    launches = g.launch_count() - l0
+    _, st = g.timestep(dP.clone(), dt, want_stats=True) if world == 1 else (None, None)
+
+    # end to end through the C ABI with HOST buffers (pinned): H2D of P, one step, D2H of P, every step
+    hP = torch.from_numpy(P0.copy()).pin_memory()
+    e2e_steps = max(1, min(args.steps, 5))
+    slab.timestep_host(hP, dt)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        slab.timestep_host(hP, dt)
+    barrier()
+    e2e_s = (time.perf_counter() - t0) / e2e_steps
+
+    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms, e2e_s = float(tmax[0]), float(tmax[1])
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    hbm_gbs, sm_max, which = peaks()
+    stages = 2 * args.steps
+    nk_ms, nk_n = timing["newton"]
+    newton_ms = nk_ms / max(nk_n, 1)
+    alu_peak = N_SM * FP64_INSTR_PER_CLK_PER_SM * sm_max * 1e6 / 1e12          # T fp64 thread-instr/s
+    alu_ach = ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON * zones / (newton_ms * 1e-3) / 1e12
+    hbm_ach = ALG_BYTES_PER_ZONE_STAGE_NEWTON * zones / (newton_ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": zones * world * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": "config3-emhd-mp5-llf-minkowski-%d^3" % n, "zones_per_gpu": zones,
+                   "update": "one zone advanced one grim_timestep = 2 stages x (ghosts, MP5+LLF fluxes, stage "
+                             "constants, fused Newton solve)", "dt": "fixed: CFL 0.5 on the initial data",
+                   "l2": "inputs (%.2f GB per field) larger than L2" % (pbytes / 1e9),
+                   "parallelism": "slab%d" % world},
+        "clocks": clocks,
+        "e2e": {"value": zones * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": pbytes,
+                "d2h_bytes_per_step": pbytes},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "alu", "kernel": "newton_stage_kernel<10,flat>", "achieved": alu_ach, "peak": alu_peak,
+                     "unit": "T fp64 instr/s", "frac": alu_ach / alu_peak, "traffic": None,
+                     "peak_source": "148 SM x 64 fp64 lanes x %s sm_max_mhz %.0f" % (which, sm_max),
+                     "launch_ms": newton_ms, "launches": int(nk_n)},
+        "roofline_hbm": {"bound": "hbm", "kernel": "newton_stage_kernel<10,flat>", "achieved": hbm_ach,
+                         "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_ach / hbm_gbs, "peak_source": which},
+        "kernel_ms_per_step": {k: v[0] / args.steps for k, v in timing.items()},
+        "newton_zone_iterations_per_s": (None if st is None else
+                                         sum(i * (st.iters_hist[0][i] + st.iters_hist[1][i]) for i in range(16))
+                                         / (2 * newton_ms * 1e-3)),
+        "paper_context": "138,000 zones/s per K20 GPU, 48,000 zones/s per 16-core node (PAPER.md L414; 64^3/device)",
+    }
+    if world == 1 and not args.no_cpu_baseline:
+        v, sps, cores = oracle_sample(args.ref_n, 2, 0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": "config-3 generator at %d^3, 2 time steps (%.1f s)" % (args.ref_n, 2 * sps)}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--n", type=int, default=256, help="zones per direction per GPU (headline 256)")
+    ap.add_argument("--ref-n", type=int, default=48, help="grid size of the oracle's bounded sample")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        if args.warmup < 3:
+            args.warmup = 3      # timing rule: at least 3 warm-up steps
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -181,6 +181,14 @@ int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, d
 /* Number of kernels the library has launched on this context since creation (host bookkeeping). */
 int64_t grim_launch_count(const grim_ctx *c);
 
+/* Per-kernel-class device timing for the roofline report (bench.py): while on, every launch group is bracketed by
+ * a CUDA event pair on the context's stream.  grim_set_timing(on != 0) clears the accumulators; grim_get_timing
+ * waits for the recorded events and returns, per class, the summed device milliseconds and the launch count
+ * (host out, GRIM_NKCLASS entries each, may be NULL).  Classes: */
+enum { GRIM_K_GHOSTS = 0, GRIM_K_FLUX = 1, GRIM_K_NEWTON = 2, GRIM_K_INVERT = 3, GRIM_K_OTHER = 4, GRIM_NKCLASS = 5 };
+int grim_set_timing(grim_ctx *c, int32_t on);
+int grim_get_timing(grim_ctx *c, double *ms, int64_t *launches);
+
 #ifdef __cplusplus
 }
 #endif

@@ -65,6 +65,9 @@ static void kerr_mks_gcov_c(double a, double h, double complex X1, double comple
   double complex r = cexp(X1);                                            /* eq 5 */
   double complex th = M_PI * X2 + 0.5 * (1.0 - h) * csin(2.0 * M_PI * X2); /* eq 6 */
   double complex sth = csin(th), cth = ccos(th);
+  /* C-21: faces on the polar axis (theta = 0, pi) have sin(theta) = 0 and a singular metric; floor |sin(theta)|
+   * at 1e-20 there, so that g^{mu nu} stays finite while sqrt(-g) ~ 1e-20 shuts the flux through the axis off */
+  if (cabs(sth) < 1e-20) sth = 1e-20;
   double complex s2 = sth * sth;
   double complex Sig = r * r + a * a * cth * cth;
   double complex f = 2.0 * r / Sig;

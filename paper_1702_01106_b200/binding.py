@@ -60,7 +60,11 @@ _SIGNATURES = {
     "grim_timestep_host": (C.c_int, [_vp, _vp, _i32, _dbl, _pd]),
     "grim_invert_primitives_host": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp]),
     "grim_launch_count": (_i64, [_vp]),
+    "grim_set_timing": (C.c_int, [_vp, _i32]),
+    "grim_get_timing": (C.c_int, [_vp, _pd, _pi64]),
 }
+
+KERNEL_CLASSES = ("ghosts", "flux", "newton", "invert", "other")
 
 
 def exported_symbols():
@@ -182,6 +186,16 @@ class Grid:
 
     def launch_count(self):
         return int(self._L.grim_launch_count(self.h))
+
+    def set_timing(self, on=True):
+        self._check(self._L.grim_set_timing(self.h, 1 if on else 0), "grim_set_timing")
+
+    def get_timing(self):
+        """{class: (device ms, launches)} accumulated since set_timing(True)."""
+        ms = (C.c_double * len(KERNEL_CLASSES))()
+        n = (C.c_int64 * len(KERNEL_CLASSES))()
+        self._check(self._L.grim_get_timing(self.h, ms, n), "grim_get_timing")
+        return {k: (ms[i], n[i]) for i, k in enumerate(KERNEL_CLASSES)}
 
     # -- the entry points ----------------------------------------------------------------------------------
     def set_metric(self, kind, params=()):

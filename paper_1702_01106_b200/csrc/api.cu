@@ -6,11 +6,17 @@
 #include <string.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/grim.h"
 #include "grim_internal.h"
 
 using namespace grim;
+
+struct KernelSpan {
+  int kclass, launches;
+  cudaEvent_t e0, e1;
+};
 
 struct grim_ctx {
   grim_grid_desc d;
@@ -34,8 +40,43 @@ struct grim_ctx {
   double *invbuf;              // U, P, resnorm, iters, status of grim_invert_primitives_host
   long long invbuf_nz;
   int64_t launches;
+  // optional per-kernel-class timing (grim_set_timing): event pairs recorded around the launches
+  int timing;
+  std::vector<KernelSpan> spans;
+  double class_ms[GRIM_NKCLASS];
+  int64_t class_n[GRIM_NKCLASS];
   std::string err;
 };
+
+// records an event pair around the launches enqueued by `body` when timing is on
+template <class F>
+static int timed(grim_ctx *c, int kclass, F body) {
+  if (!c->timing) return body();
+  KernelSpan sp;
+  sp.kclass = kclass;
+  cudaEventCreate(&sp.e0);
+  cudaEventCreate(&sp.e1);
+  cudaEventRecord(sp.e0, c->stream);
+  int n = body();
+  cudaEventRecord(sp.e1, c->stream);
+  sp.launches = n;
+  c->spans.push_back(sp);
+  return n;
+}
+
+static void drain_spans(grim_ctx *c) {
+  for (auto &sp : c->spans) {
+    cudaEventSynchronize(sp.e1);
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, sp.e0, sp.e1) == cudaSuccess) {
+      c->class_ms[sp.kclass] += ms;
+      c->class_n[sp.kclass] += sp.launches;
+    }
+    cudaEventDestroy(sp.e0);
+    cudaEventDestroy(sp.e1);
+  }
+  c->spans.clear();
+}
 
 static std::string g_init_error;
 
@@ -65,6 +106,27 @@ extern "C" const char *grim_last_error(const grim_ctx *c) { return c ? c->err.c_
 
 extern "C" int64_t grim_launch_count(const grim_ctx *c) { return c ? c->launches : 0; }
 
+extern "C" int grim_set_timing(grim_ctx *c, int32_t on) {
+  if (!c) return GRIM_EINVAL;
+  cudaSetDevice(c->d.device);
+  drain_spans(c);
+  c->timing = on ? 1 : 0;
+  if (on)
+    for (int k = 0; k < GRIM_NKCLASS; k++) { c->class_ms[k] = 0.0; c->class_n[k] = 0; }
+  return GRIM_OK;
+}
+
+extern "C" int grim_get_timing(grim_ctx *c, double *ms, int64_t *launches) {
+  if (!c) return GRIM_EINVAL;
+  cudaSetDevice(c->d.device);
+  drain_spans(c);
+  for (int k = 0; k < GRIM_NKCLASS; k++) {
+    if (ms) ms[k] = c->class_ms[k];
+    if (launches) launches[k] = c->class_n[k];
+  }
+  return GRIM_OK;
+}
+
 extern "C" int64_t grim_zones_padded(const grim_ctx *c, int32_t extents[3]) {
   if (!c) return 0;
   if (extents)
@@ -76,6 +138,7 @@ extern "C" void grim_free(grim_ctx *c) {
   if (!c) return;
   cudaSetDevice(c->d.device);
   cudaStreamSynchronize(c->stream);
+  drain_spans(c);
   void *ptrs[] = {c->geomC, c->geomF[0], c->geomF[1], c->geomF[2], c->conn, c->C, c->G, c->Fface, c->cface,
                   c->Ph, c->Pnew, c->resnorm, c->status, c->iters, c->cnt, c->stats, c->probe_sink,
                   c->list[0], c->list[1], c->hostP, c->invbuf};
@@ -123,6 +186,8 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   c->stream = (cudaStream_t)d->stream;
   c->metric_set = 0;
   c->launches = 0;
+  c->timing = 0;
+  for (int k = 0; k < GRIM_NKCLASS; k++) { c->class_ms[k] = 0.0; c->class_n[k] = 0; }
   GridView &gv = c->gv;
   memset(&gv, 0, sizeof(gv));
   gv.dim = d->dim;
@@ -193,12 +258,12 @@ extern "C" int grim_set_metric(grim_ctx *c, int32_t kind, const double *params, 
   if (!c) return GRIM_EINVAL;
   CU(cudaSetDevice(c->d.device));
   if (kind == GRIM_MINKOWSKI) {
-    c->launches += launch_metric_flat(c->gv, c->geomC, c->geomF[0], c->geomF[1], c->geomF[2], c->conn, c->stream);
+    c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_metric_flat(c->gv, c->geomC, c->geomF[0], c->geomF[1], c->geomF[2], c->conn, c->stream); });
   } else if (kind == GRIM_KERR_MKS) {
     if (!params || nparams < 2) return fail(c, GRIM_EINVAL, "Kerr needs params = {a, h}");
     if (c->d.dim < 2) return fail(c, GRIM_EINVAL, "Kerr needs at least the X1, X2 directions");
-    c->launches += launch_metric_kerr(c->gv, params[0], params[1], c->d.tau_mode, c->geomC, c->geomF[0],
-                                      c->geomF[1], c->geomF[2], c->conn, c->stream);
+    c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_metric_kerr(c->gv, params[0], params[1], c->d.tau_mode, c->geomC, c->geomF[0],
+                                      c->geomF[1], c->geomF[2], c->conn, c->stream); });
   } else {
     return fail(c, GRIM_EINVAL, "unknown metric");
   }
@@ -218,7 +283,7 @@ static int need_metric(grim_ctx *c) {
 extern "C" int grim_fill_ghosts(grim_ctx *c, double *P) {
   if (!c || !P) return fail(c, GRIM_EINVAL, "grim_fill_ghosts: null argument");
   CU(cudaSetDevice(c->d.device));
-  c->launches += launch_fill_ghosts(c->gv, c->d.bc, P, c->stream);
+  c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(c->gv, c->d.bc, P, c->stream); });
   return check_launch(c, "fill_ghosts kernel");
 }
 
@@ -234,8 +299,8 @@ extern "C" int grim_compute_fluxes(grim_ctx *c, const double *P_E, const double 
     CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
     cnt = c->cnt;
   }
-  c->launches += launch_fluxes(c->gv, P_E, P_n, dt_stage, C_out ? C_out : c->C, G_out ? G_out : c->G, c->Fface,
-                               c->cface, cnt, c->stream);
+  c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(c->gv, P_E, P_n, dt_stage, C_out ? C_out : c->C, G_out ? G_out : c->G, c->Fface,
+                               c->cface, cnt, c->stream); });
   rc = check_launch(c, "flux kernels");
   if (rc) return rc;
   if (speeds_out)
@@ -253,8 +318,8 @@ extern "C" int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_
   if (!(dt_stage > 0.0)) return fail(c, GRIM_EINVAL, "dt_stage must be positive");
   CU(cudaSetDevice(c->d.device));
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
-  c->launches += launch_newton_stage(c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, dt_stage, max_iters, P_iter,
-                                     resnorm, status, iters, c->cnt, c->stream);
+  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, dt_stage, max_iters, P_iter,
+                                     resnorm, status, iters, c->cnt, c->stream); });
   rc = check_launch(c, "newton_stage kernel");
   if (rc) return rc;
   if (n_active_out) {
@@ -269,7 +334,7 @@ extern "C" int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_
 extern "C" int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, double *U) {
   if (!c || !P || !U || nz < 0) return fail(c, GRIM_EINVAL, "grim_prim_to_conserved: bad argument");
   CU(cudaSetDevice(c->d.device));
-  c->launches += launch_prim_to_conserved(c->gv, nz, P, U, c->stream);
+  c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_prim_to_conserved(c->gv, nz, P, U, c->stream); });
   return check_launch(c, "prim_to_conserved kernel");
 }
 
@@ -296,8 +361,8 @@ extern "C" int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_t
   while (nlist > 0) {
     const int sweep = first ? 4 : 2;
     CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
-    c->launches += launch_invert(c->gv, nz, nlist, c->list[cur], U_target, P_inout, iters, status, resnorm, sweep,
-                                 first, c->list[cur ^ 1], c->cnt, c->stream);
+    c->launches += timed(c, GRIM_K_INVERT, [&] { return launch_invert(c->gv, nz, nlist, c->list[cur], U_target, P_inout, iters, status, resnorm, sweep,
+                                 first, c->list[cur ^ 1], c->cnt, c->stream); });
     int rc = check_launch(c, "invert kernel");
     if (rc) return rc;
     unsigned long long cntn = 0;
@@ -330,11 +395,11 @@ extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used,
   cudaStream_t s = c->stream;
   unsigned long long bt[2] = {0, 0};
 
-  c->launches += launch_fill_ghosts(gv, c->d.bc, P, s);
+  c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(gv, c->d.bc, P, s); });
   if (!(dt > 0.0)) {
     // C-15: dt = cfl / max_z sum_d c^d/dX^d, from a flux pass over P_n
     CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
-    c->launches += launch_fluxes(gv, P, P, 1.0, c->C, c->G, c->Fface, c->cface, c->cnt, s);
+    c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, P, P, 1.0, c->C, c->G, c->Fface, c->cface, c->cnt, s); });
     double sp3 = 0.0;
     CU(cudaMemcpyAsync(&sp3, &c->cnt->speeds[3], sizeof(double), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
@@ -345,28 +410,28 @@ extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used,
 
   // stage 1: P_E = P_n, dt' = dt/2, guess P_n (eq 19; C-7)
   const double dt1 = 0.5 * dt;
-  c->launches += launch_fluxes(gv, P, P, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s);
+  c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, P, P, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s); });
   CU(cudaMemcpyAsync(c->Ph, P, pbytes, cudaMemcpyDeviceToDevice, s));
   CU(cudaMemsetAsync(c->status, 0, (size_t)gv.zg * 4, s));
   CU(cudaMemsetAsync(c->iters, 0, (size_t)gv.zg * 4, s));
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
-  c->launches += launch_newton_stage(gv, P, P, c->C, c->G, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s);
+  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, P, c->C, c->G, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s); });
   if (stats) {
-    c->launches += launch_stats(gv, P, dt1, c->resnorm, c->status, c->iters, &c->stats[0], s);
+    c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_stats(gv, P, dt1, c->resnorm, c->status, c->iters, &c->stats[0], s); });
     CU(cudaMemcpyAsync(&bt[0], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));
   }
   // stage 2: P_E = P_{n+1/2}, dt' = dt, guess P_{n+1/2} (eq 13)
-  c->launches += launch_fill_ghosts(gv, c->d.bc, c->Ph, s);
-  c->launches += launch_fluxes(gv, c->Ph, P, dt, c->C, c->G, c->Fface, c->cface, nullptr, s);
+  c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(gv, c->d.bc, c->Ph, s); });
+  c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, c->Ph, P, dt, c->C, c->G, c->Fface, c->cface, nullptr, s); });
   CU(cudaMemcpyAsync(c->Pnew, c->Ph, pbytes, cudaMemcpyDeviceToDevice, s));
   CU(cudaMemsetAsync(c->status, 0, (size_t)gv.zg * 4, s));
   CU(cudaMemsetAsync(c->iters, 0, (size_t)gv.zg * 4, s));
   if (stats) CU(cudaStreamSynchronize(s));  // bt[0] must land before the counters are cleared
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
-  c->launches += launch_newton_stage(gv, P, c->Ph, c->C, c->G, dt, 0, c->Pnew, c->resnorm, c->status, c->iters,
-                                     c->cnt, s);
+  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, c->Ph, c->C, c->G, dt, 0, c->Pnew, c->resnorm, c->status, c->iters,
+                                     c->cnt, s); });
   if (stats) {
-    c->launches += launch_stats(gv, P, dt, c->resnorm, c->status, c->iters, &c->stats[1], s);
+    c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_stats(gv, P, dt, c->resnorm, c->status, c->iters, &c->stats[1], s); });
     CU(cudaMemcpyAsync(&bt[1], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));
   }
   CU(cudaMemcpyAsync(P, c->Pnew, pbytes, cudaMemcpyDeviceToDevice, s));

@@ -46,6 +46,7 @@ __device__ void kerr_mks_gcov(double a, double h, double X1, double X2, Dual (&g
   Dual r = dexp(x1);                                                  // eq 5
   Dual th = pi * x2 + (0.5 * (1.0 - h)) * dsin((2.0 * pi) * x2);       // eq 6
   Dual sth = dsin(th), cth = dcos(th);
+  if (fabs(sth.v) < 1e-20) sth = dmake(1e-20);  // C-21: faces on the polar axis; keeps g^{mu nu} finite, sqrt(-g) ~ 0
   Dual s2 = sth * sth;
   Dual Sig = r * r + (a * a) * (cth * cth);
   Dual f = (2.0 * r) / Sig;

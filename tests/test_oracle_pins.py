@@ -260,3 +260,18 @@ def test_kerr_a0_is_schwarzschild_ingoing():
 def test_minkowski_geometry():
     gcov, gcon, sg, alpha = og.geom_arrays(og.minkowski())
     assert np.array_equal(gcov, np.diag([-1.0, 1, 1, 1])) and np.array_equal(gcon, gcov) and sg == 1 and alpha == 1
+
+
+def test_kerr_polar_axis_face_is_finite():
+    """C-21: on a face lying on the polar axis (X2 = 0 or 1) sin(theta) = 0 and the metric is singular; the floor
+    |sin theta| >= 1e-20 keeps g^{mu nu} finite (g g^-1 = 1 still holds) while sqrt(-g) ~ 1e-20 shuts the flux
+    through the axis off.  Away from the axis the floor is inactive (bit-identical metric)."""
+    for X2 in (0.0, 1.0):
+        g = og.kerr_mks(0.9375, 0.3, np.log(5.0), X2)
+        gcov, gcon, sg, al = og.geom_arrays(g)
+        assert np.isfinite(gcov).all() and np.isfinite(gcon).all() and np.isfinite(al)
+        assert 0.0 < sg < 1e-12      # X2 = 1: sin(pi) = 1.2e-16 in fp64, already non-zero; X2 = 0: the floor
+        I = gcov @ gcon
+        assert abs(I - np.eye(4)).max() < 1e-12
+    g1 = og.geom_arrays(og.kerr_mks(0.9375, 0.3, np.log(5.0), 1e-3))
+    assert g1[2] > 1e-3      # floor inactive: sqrt(-g) = Sigma sin(theta) |det L| is of order r^3 * 2 pi X2
