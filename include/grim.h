@@ -160,6 +160,17 @@ int grim_fill_ghosts(grim_ctx *c, double *P);
 /* U(P) for nz flat zones, Minkowski (eqs 30-32, 39-42); used to build inversion workloads on the device. */
 int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, double *U);
 
+/* Caller-supplied stationary metric independent of X^3 (the paper keeps geometry in a separate library, L339):
+ * replaces the tables grim_set_metric would compute.  Both arguments HOST, SoA over the padded 2-D plane
+ * idx2d = j*s1 + i (n2d = s1*s2 entries per component):
+ *   tab  : [loc][comp][idx2d], loc = 0 centre, 1..3 lower face in direction loc; comp 0..9 = g_mu_nu in the
+ *          order 00 01 02 03 11 12 13 22 23 33, 10..19 = g^mu^nu (same order), 20 = sqrt(-g), 21 = lapse,
+ *          22 = tau_R (used when tau_mode == GRIM_TAU_R32; otherwise the descriptor's tau)      (4*23*n2d doubles)
+ *   conn : [l*16 + m*4 + n][idx2d] = Gamma^l_{mn} at zone centres                                (64*n2d doubles)
+ * The library derives alpha g^{ti} (one multiplication per entry) and copies the rest unchanged.  Afterwards the
+ * context behaves as after grim_set_metric(GRIM_KERR_MKS): general-metric kernels.  Synchronises. */
+int grim_set_metric_tables(grim_ctx *c, const double *tab, const double *conn);
+
 /* Copies the geometry of padded 2-D zone (j,i) -> idx2d = j*s1 + i to the HOST (parity tests of a0):
  * loc = 0 centre, 1..3 lower face in direction loc.  gcov, gcon: 16 doubles row-major; conn: 64 doubles
  * [l][m][n] = Gamma^l_{mn} (centre only; may be NULL).  Synchronises. */

@@ -596,6 +596,9 @@ void og_grid_get_geom(const og_grid *g, int loc, int64_t idx2d, og_geom *out) {
 void og_grid_get_conn(const og_grid *g, int64_t idx2d, double conn[4][4][4]) {
   memcpy(conn, g->conn[idx2d], sizeof(double[4][4][4]));
 }
+double og_grid_get_tau(const og_grid *g, int loc, int64_t idx2d) {
+  return (loc == 0) ? g->tauC[idx2d] : g->tauF[loc - 1][idx2d];
+}
 
 /* Ghost fill (C-11): periodic / outflow (copy) / polar reflection (sign flip of the X2 components) / none.
  * Direction 1 first, then 2 (covering direction-1 ghosts), then 3. */

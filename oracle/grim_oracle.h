@@ -123,6 +123,7 @@ void     og_fill_ghosts(const og_grid *g, double *P);
 /* geometry tables as the oracle holds them (for the geometry parity test): padded 2-D [j][i] */
 void     og_grid_get_geom(const og_grid *g, int loc /*0 centre,1..3 lower faces*/, int64_t idx2d, og_geom *out);
 void     og_grid_get_conn(const og_grid *g, int64_t idx2d, double conn[4][4][4]);
+double   og_grid_get_tau(const og_grid *g, int loc, int64_t idx2d);   /* tau_R of that evaluation point (C-11) */
 /* stage constant C (nvar x Zg) and explicit EMHD gradient terms G (3 x Zg: Xq, Xd, divx) (L438).
    speeds[0..2] = max_z c^d/dX^d, speeds[3] = max_z sum_d c^d/dX^d */
 void     og_stage_prepare(const og_grid *g, const double *Pn, const double *PE, double dt_stage,

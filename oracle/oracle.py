@@ -104,6 +104,8 @@ def _declare(L):
     L.og_fill_ghosts.argtypes = [C.c_void_p, _dp]
     L.og_grid_get_geom.argtypes = [C.c_void_p, C.c_int, C.c_int64, C.POINTER(Geom)]
     L.og_grid_get_conn.argtypes = [C.c_void_p, C.c_int64, _dp]
+    L.og_grid_get_tau.argtypes = [C.c_void_p, C.c_int, C.c_int64]
+    L.og_grid_get_tau.restype = C.c_double
     L.og_stage_prepare.argtypes = [C.c_void_p, _dp, _dp, C.c_double, _dp, _dp, _dp]
     L.og_zone_residual.argtypes = [C.c_void_p, C.c_int64, _dp, _dp, _dp, _dp, C.c_double, _dp, _dp]
     L.og_newton.argtypes = [C.c_void_p, _dp, _dp, _dp, _dp, C.c_double, _dp, C.c_int, _dp, _ip, _ip,
@@ -335,6 +337,32 @@ class Grid:
         out = np.zeros((4, 4, 4))
         lib().og_grid_get_conn(self.h, j * self.sz[0] + i, _d(out))
         return out
+
+    def tau(self, loc, j, i):
+        return lib().og_grid_get_tau(self.h, loc, j * self.sz[0] + i)
+
+    def geometry_tables(self):
+        """The grid's geometry as plain tables over the padded 2-D plane (idx2d = j*s1 + i), in the layout of
+        include/grim.h grim_set_metric_tables: tab[loc][comp][idx2d] with comp 0..9 = g_mu_nu (00 01 02 03 11 12 13
+        22 23 33), 10..19 = g^mu^nu, 20 = sqrt(-g), 21 = lapse, 22 = tau_R; conn[l*16 + m*4 + n][idx2d].  Copies
+        of stored values only (no arithmetic)."""
+        n2d = self.sz[0] * self.sz[1]
+        tab = np.zeros((4, 23, n2d))
+        conn = np.zeros((64, n2d))
+        sym = [(0, 0), (0, 1), (0, 2), (0, 3), (1, 1), (1, 2), (1, 3), (2, 2), (2, 3), (3, 3)]
+        for j in range(self.sz[1]):
+            for i in range(self.sz[0]):
+                id2 = j * self.sz[0] + i
+                for loc in range(4):
+                    g = self.geom(loc, j, i)
+                    for c, (m, n) in enumerate(sym):
+                        tab[loc, c, id2] = g.gcov[m][n]
+                        tab[loc, 10 + c, id2] = g.gcon[m][n]
+                    tab[loc, 20, id2] = g.sqrtmg
+                    tab[loc, 21, id2] = g.alpha
+                    tab[loc, 22, id2] = self.tau(loc, j, i)
+                conn[:, id2] = self.conn(j, i).reshape(64)
+        return tab, conn
 
     def stage_prepare(self, Pn, PE, dt_stage):
         Cc = np.zeros(self.shape)

@@ -45,6 +45,7 @@ _pd, _pi32, _pi64 = C.POINTER(C.c_double), C.POINTER(C.c_int32), C.POINTER(C.c_i
 _SIGNATURES = {
     "grim_init_grid": (C.c_int, [C.POINTER(_vp), C.POINTER(GridDesc)]),
     "grim_set_metric": (C.c_int, [_vp, _i32, _pd, _i32]),
+    "grim_set_metric_tables": (C.c_int, [_vp, _pd, _pd]),
     "grim_compute_fluxes": (C.c_int, [_vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "grim_newton_step": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _i32, _vp, _vp, _vp, _vp, _pi64]),
     "grim_invert_primitives": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
@@ -201,6 +202,17 @@ class Grid:
     def set_metric(self, kind, params=()):
         arr = (C.c_double * max(len(params), 1))(*[float(x) for x in params])
         self._check(self._L.grim_set_metric(self.h, kind, arr, len(params)), "grim_set_metric")
+
+    def set_metric_tables(self, tab, conn):
+        """tab: numpy float64 [4, 23, n2d]; conn: [64, n2d] (layout: include/grim.h)."""
+        import numpy as np
+        n2d = self.sz[0] * self.sz[1]
+        tab = np.ascontiguousarray(tab, dtype=np.float64)
+        conn = np.ascontiguousarray(conn, dtype=np.float64)
+        if tab.shape != (4, 23, n2d) or conn.shape != (64, n2d):
+            raise GrimError("set_metric_tables: expected shapes (4, 23, %d) and (64, %d)" % (n2d, n2d))
+        self._check(self._L.grim_set_metric_tables(self.h, tab.ctypes.data_as(_pd), conn.ctypes.data_as(_pd)),
+                    "grim_set_metric_tables")
 
     def fill_ghosts(self, P):
         self._check(self._L.grim_fill_ghosts(self.h, _ptr(P, self.torch.float64)), "grim_fill_ghosts")

@@ -274,6 +274,34 @@ extern "C" int grim_set_metric(grim_ctx *c, int32_t kind, const double *params, 
   return GRIM_OK;
 }
 
+extern "C" int grim_set_metric_tables(grim_ctx *c, const double *tab, const double *conn) {
+  if (!c) return GRIM_EINVAL;
+  if (!tab || !conn) return fail(c, GRIM_EINVAL, "grim_set_metric_tables: null argument");
+  if (c->d.dim < 2) return fail(c, GRIM_EINVAL, "a general metric needs at least the X1, X2 directions");
+  CU(cudaSetDevice(c->d.device));
+  const size_t n2d = (size_t)c->gv.n2d;
+  std::vector<double> h((size_t)GT_NCOMP * n2d);
+  for (int loc = 0; loc < 4; loc++) {
+    const double *t = tab + (size_t)loc * 23 * n2d;
+    memcpy(&h[(size_t)GT_GCOV * n2d], t, 20 * n2d * sizeof(double));  // g_mu_nu, g^mu^nu
+    memcpy(&h[(size_t)GT_SQRTMG * n2d], t + 20 * n2d, n2d * sizeof(double));
+    memcpy(&h[(size_t)GT_ALPHA * n2d], t + 21 * n2d, n2d * sizeof(double));
+    for (size_t id = 0; id < n2d; id++) {
+      h[(size_t)GT_TAU * n2d + id] = (c->d.tau_mode == GRIM_TAU_R32) ? t[22 * n2d + id] : c->d.tau;
+      for (int i = 1; i < 4; i++)  // alpha g^{ti} = beta^i/alpha (C-9)
+        h[(size_t)(GT_BFAC + i - 1) * n2d + id] = t[21 * n2d + id] * t[(size_t)(GT_GCON + sym4(0, i)) * n2d + id];
+    }
+    double *dst = loc == 0 ? c->geomC : c->geomF[loc - 1];
+    CU(cudaMemcpyAsync(dst, h.data(), h.size() * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+  }
+  CU(cudaMemcpyAsync(c->conn, conn, (size_t)CONN_NCOMP * n2d * sizeof(double), cudaMemcpyHostToDevice, c->stream));
+  CU(cudaStreamSynchronize(c->stream));
+  c->gv.metric = GRIM_KERR_MKS;
+  c->metric_set = 1;
+  return GRIM_OK;
+}
+
 static int need_metric(grim_ctx *c) {
   if (!c) return GRIM_EINVAL;
   if (!c->metric_set) return fail(c, GRIM_ESTATE, "grim_set_metric has not been called");

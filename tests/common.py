@@ -37,13 +37,20 @@ def to_dev(a, dtype=None):
     return t if dtype is None else t.to(dtype)
 
 
-def rel_err_per_primitive(A, B, interior=None):
+def rel_err_per_primitive(A, B, interior=None, gam=None):
     """north_star metric: max over zones of |A-B| / max(|B|, floor_v), floor_v = 1e-12 max_z|B_v|; velocity and
-    field components relative to the norm of their vector."""
+    field components relative to the norm of their vector.  With gam given, q and dP (which change
+    sign and pass through zero inside the domain) are measured against max(|q|, 1e-3 rho Theta^{3/2}) and
+    max(|dP|, 1e-3 P_g): a thousandth of their free-streaming / isotropic-pressure scale."""
     if interior is not None:
         A, B = interior(A), interior(B)
     nv = A.shape[0]
     out = np.zeros(nv)
+    if gam is not None and nv == 10:
+        pg = (gam - 1.0) * abs(B[1])
+        nat = {8: 1e-3 * abs(B[0]) * (pg / abs(B[0])) ** 1.5, 9: 1e-3 * pg}
+    else:
+        nat = {}
     def vecnorm(X, lo):
         return np.sqrt((X[lo:lo + 3] ** 2).sum(axis=0))
     for v in range(nv):
@@ -54,6 +61,8 @@ def rel_err_per_primitive(A, B, interior=None):
         else:
             ref = abs(B[v])
         floor = 1e-12 * max(ref.max(), 1e-300)
+        if v in nat:
+            ref = np.maximum(ref, nat[v])
         out[v] = (abs(A[v] - B[v]) / np.maximum(ref, floor)).max()
     return out
 

@@ -38,10 +38,12 @@ def test_config3_fullsize_sampled(n):
     P1 = gc.interior(dP).cpu().numpy()
     del dP
     assert st.unconverged[0] == 0 and st.unconverged[1] == 0
-    # 2 iterations per stage (C-13), except the few zones per million whose round-off floor after the second
-    # iteration sits above rtol * scale and that take a third
+    # 2 iterations per stage (C-13), except for the ~1e-4 of the zones on either side of the threshold: those whose
+    # residual after the first iteration is already below rtol * scale, and those whose round-off floor after the
+    # second sits above it and that take a third (the sampled zones below are compared with the oracle bit by bit)
     for s in range(2):
-        assert st.iters_hist[s][2] + st.iters_hist[s][3] == n ** 3 and st.iters_hist[s][3] < 1e-3 * n ** 3
+        h = st.iters_hist[s]
+        assert h[1] + h[2] + h[3] == n ** 3 and h[2] > 0.999 * n ** 3
     rng = np.random.default_rng(n)
     cs = [tuple(rng.integers(0, n, 3)) for _ in range(40)]
     cs += [(0, 0, 0), (n - 1, n - 1, n - 1), (0, n - 1, 5), (n // 2, 0, n - 1)]          # wrap-around corners
