@@ -86,7 +86,7 @@ stage_const_kernel(GridView gv, const double *__restrict__ PE, const double *__r
     zone_coords(gv, t, i, j, k);
     const long long z = zone_index(gv, i, j, k);
     const long long id = (long long)j * gv.sz[0] + i;
-    const double idt = 1.0 / dt_stage;
+    const double idt = drcp(dt_stage);
     G gc;
     double tau = gv.tau_const;
     if constexpr (!G::flat) load_geom<0>(gv.geomC, gv.n2d, id, gc, tau);
@@ -183,8 +183,8 @@ stage_const_kernel(GridView gv, const double *__restrict__ PE, const double *__r
         Vel vm_, vp_;
         vel_state(gm, Pm_[U1], Pm_[U2], Pm_[U3], vm_);
         vel_state(gp, Pp_[U1], Pp_[U2], Pp_[U3], vp_);
-        const double Thm = (gv.m.gm1 * Pm_[UU]) / Pm_[RHO];
-        const double Thp = (gv.m.gm1 * Pp_[UU]) / Pp_[RHO];
+        const double Thm = ddiv(gv.m.gm1 * Pm_[UU], Pm_[RHO]);
+        const double Thp = ddiv(gv.m.gm1 * Pp_[UU], Pp_[RHO]);
         dTheta[a + 1] = limited_slope(th, Thm, sE.th.Th, Thp) * gv.idx[a];
 #pragma unroll
         for (int nu = 0; nu < 4; nu++)
@@ -196,7 +196,7 @@ stage_const_kernel(GridView gv, const double *__restrict__ PE, const double *__r
                             gv.idx[a];
         }
       }
-      if constexpr (!G::flat) divx = divx / gc.sqrtmg();
+      if constexpr (!G::flat) divx = ddiv(divx, gc.sqrtmg());
       // Xq = bhat^i d_i Theta + Theta bhat^mu (u^i d_i u_mu - Gamma^l_{nu mu} u^nu u_l)
       // Xd = bhat^i bhat^nu d_i u_nu - Gamma^l_{mu nu} bhat^mu bhat^nu u_l
       const double *bh = sE.h.con;

@@ -88,7 +88,7 @@ __device__ __forceinline__ void fd_column(const Prob &prob, const SolverParams &
   double pj = (fabs(P[J]) < 5.0 * sp.fd_eps) ? sp.fd_eps : (1.0 + sp.fd_eps) * P[J];
   double h = pj - P[J];
   if (h == 0.0) singular = true;
-  double ih = 1.0 / h;
+  double ih = drcp(h);
   double Rt[N];
   eval_column<J, N>(prob, P, pj, base, Rt);
 #pragma unroll
@@ -154,7 +154,7 @@ __device__ __forceinline__ bool lu_solve(const JacView<N, BLOCK> &jac, double (&
         int o = rowoff[j]; rowoff[j] = rowoff[i]; rowoff[i] = o;
       }
     }
-    double r = 1.0 / x[j];
+    double r = drcp(x[j]);
     rinv[j] = r;
 #pragma unroll
     for (int i = j + 1; i < N; i++) x[i] = x[i] * r;
@@ -174,7 +174,7 @@ __device__ __forceinline__ bool lu_solve(const JacView<N, BLOCK> &jac, double (&
 
 // eq 25 (L230): minimiser of the quadratic through f(0), f'(0) = -2 f(0), f(lam)
 __device__ __forceinline__ double linesearch_lambda(double f0, double flam, double lam) {
-  return f0 / (flam + (2.0 * lam - 1.0) * f0) * lam * lam;
+  return ddiv(f0, flam + (2.0 * lam - 1.0) * f0) * lam * lam;
 }
 
 // Runs at most max_iters further Newton iterations (<= 0: until terminal) of one zone.  P, iters, status carry
@@ -190,9 +190,9 @@ __device__ __forceinline__ double newton_zone(const Prob &prob, const SolverPara
   double f0 = norm2sq<N>(R0);
   if (!isfinite(f0)) {
     status = st | ST_NONFINITE;
-    return sqrt(f0);
+    return dsqrt(f0);
   }
-  while (!(sqrt(f0) < tol) && k < sp.kmax && (max_iters <= 0 || done < max_iters)) {
+  while (!(dsqrt(f0) < tol) && k < sp.kmax && (max_iters <= 0 || done < max_iters)) {
     bool singular = false;
     FdColumns<0, N, BLOCK, Prob>::run(prob, sp, P, pc, R0, jac, singular);
     double dP[N];
@@ -211,7 +211,7 @@ __device__ __forceinline__ double newton_zone(const Prob &prob, const SolverPara
       for (int v = 0; v < N; v++) Pt[v] = P[v] + lam * dP[v];
       eval_full<N>(prob, Pt, pc, Rt);
       ft = norm2sq<N>(Rt);
-      if (sqrt(ft) < sqrt(f0) * (1.0 - sp.eps_bt * lam)) {
+      if (dsqrt(ft) < dsqrt(f0) * (1.0 - sp.eps_bt * lam)) {
         accepted = true;
         break;
       }
@@ -234,12 +234,12 @@ __device__ __forceinline__ double newton_zone(const Prob &prob, const SolverPara
     }
   }
   if (!(st & (ST_SINGULAR | ST_NONFINITE))) {
-    if (sqrt(f0) < tol) st |= ST_CONVERGED;
+    if (dsqrt(f0) < tol) st |= ST_CONVERGED;
     else if (k >= sp.kmax) st |= ST_KMAX;
   }
   iters = k;
   status = st;
-  return sqrt(f0);
+  return dsqrt(f0);
 }
 
 }  // namespace grim

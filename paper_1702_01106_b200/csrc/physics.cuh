@@ -14,6 +14,8 @@
 #include <cuda_runtime.h>
 #include <math.h>
 
+#include "fp64ops.cuh"
+
 namespace grim {
 
 enum { RHO = 0, UU = 1, U1 = 2, U2 = 3, U3 = 4, B1 = 5, B2 = 6, B3 = 7, QQ = 8, DPP = 9 };
@@ -91,7 +93,7 @@ __device__ __forceinline__ void vel_state(const G &g, double ut1, double ut2, do
     double usq = ut1 * ut1;
     usq = usq + ut2 * ut2;
     usq = usq + ut3 * ut3;
-    double W = sqrt(1.0 + usq);
+    double W = dsqrt(1.0 + usq);
     v.ucon[0] = W;
     v.ucon[1] = ut1;
     v.ucon[2] = ut2;
@@ -103,8 +105,8 @@ __device__ __forceinline__ void vel_state(const G &g, double ut1, double ut2, do
     for (int i = 1; i < 4; i++)
 #pragma unroll
       for (int j = 1; j < 4; j++) usq = usq + g.cov(i, j) * ut[i - 1] * ut[j - 1];
-    double W = sqrt(1.0 + usq);
-    v.ucon[0] = W / g.alpha;
+    double W = dsqrt(1.0 + usq);
+    v.ucon[0] = ddiv(W, g.alpha);
 #pragma unroll
     for (int i = 1; i < 4; i++) v.ucon[i] = ut[i - 1] - W * g.bfac[i - 1];
   }
@@ -118,7 +120,7 @@ __device__ __forceinline__ void mag_state(const G &g, const Vel &v, double Bx, d
   bt = bt + By * v.ucov[2];
   bt = bt + Bz * v.ucov[3];
   b.bcon[0] = bt;
-  double iut = 1.0 / v.ucon[0];
+  double iut = drcp(v.ucon[0]);
   b.bcon[1] = (Bx + bt * v.ucon[1]) * iut;
   b.bcon[2] = (By + bt * v.ucon[2]) * iut;
   b.bcon[3] = (Bz + bt * v.ucon[3]) * iut;
@@ -131,7 +133,7 @@ __device__ __forceinline__ void mag_state(const G &g, const Vel &v, double Bx, d
 }
 
 __device__ __forceinline__ void bhat_state(const Mag &b, BHat &h) {
-  double ibn = 1.0 / sqrt(b.bsq);
+  double ibn = drcp(dsqrt(b.bsq));
 #pragma unroll
   for (int i = 0; i < 4; i++) {
     h.con[i] = b.bcon[i] * ibn;
@@ -142,7 +144,7 @@ __device__ __forceinline__ void bhat_state(const Mag &b, BHat &h) {
 // c_s^2 = gam P_g/(rho + gam u) (eq 45; L501)
 __device__ __forceinline__ double sound_speed2(const ModelParams &m, double rho, double u) {
   double Pg = m.gm1 * u;
-  return m.gam * Pg / (rho + m.gam * u);
+  return ddiv(m.gam * Pg, rho + m.gam * u);
 }
 
 // eqs 41-42 (L291-293): q~ = q sqrt(tau/(chi rho Theta^2)), dP~ = dP sqrt(tau/(nu rho Theta)), closure of the
@@ -151,12 +153,12 @@ template <int N>
 __device__ __forceinline__ void thermo_state(const ModelParams &m, double tau, double rho, double u, Thermo &t) {
   t.Pg = m.gm1 * u;
   if constexpr (N == 10) {
-    t.Th = t.Pg / rho;
-    double cs2 = m.gam * t.Pg / (rho + m.gam * u);
+    t.Th = ddiv(t.Pg, rho);
+    double cs2 = ddiv(m.gam * t.Pg, rho + m.gam * u);
     double chi = m.phi * cs2 * tau;
     double nu = m.psi * cs2 * tau;
-    t.fq = sqrt(tau / (chi * rho * t.Th * t.Th));
-    t.fdp = sqrt(tau / (nu * rho * t.Th));
+    t.fq = dsqrt(ddiv(tau, chi * rho * t.Th * t.Th));
+    t.fdp = dsqrt(ddiv(tau, nu * rho * t.Th));
   } else {
     t.Th = 0.0;
     t.fq = 0.0;
@@ -237,13 +239,13 @@ __device__ __forceinline__ void full_state(const ModelParams &m, const G &g, dou
 template <int N>
 __device__ __forceinline__ double vmax2(const ModelParams &m, double tau, double rho, double u, double bsq) {
   double cs2 = sound_speed2(m, rho, u);
-  double va2 = bsq / (rho + m.gam * u + bsq);
+  double va2 = ddiv(bsq, rho + m.gam * u + bsq);
   double cst2 = cs2;
   if constexpr (N == 10) {
     double chi = m.phi * cs2 * tau, nu = m.psi * cs2 * tau;
-    double vq2 = m.gm1 * chi / tau;
-    double vdp2 = 4.0 * nu / (3.0 * tau);
-    cst2 = 0.5 * (cs2 + vq2 + sqrt(cs2 * cs2 + vq2 * vq2)) + vdp2;
+    double vq2 = ddiv(m.gm1 * chi, tau);
+    double vdp2 = ddiv(4.0 * nu, 3.0 * tau);
+    cst2 = 0.5 * (cs2 + vq2 + dsqrt(cs2 * cs2 + vq2 * vq2)) + vdp2;
   }
   return cst2 + va2 - cst2 * va2;
 }
@@ -265,8 +267,8 @@ __device__ __forceinline__ double cmax_dir(const G &g, double vm2, double ut, do
   double A = ut * ut - (g00 + ut * ut) * vm2;
   double B = 2.0 * (ud * ut - (g0d + ud * ut) * vm2);
   double C = ud * ud - (gdd + ud * ud) * vm2;
-  double disc = sqrt(fmax(B * B - 4.0 * A * C, 0.0));
-  double i2A = 1.0 / (2.0 * A);
+  double disc = dsqrt(fmax(B * B - 4.0 * A * C, 0.0));
+  double i2A = drcp(2.0 * A);
   double vp = (B + disc) * i2A;
   double vn = (B - disc) * i2A;
   return fmax(fabs(vp), fabs(vn));

@@ -27,13 +27,13 @@ struct StageProblem {
 
   // Everything that depends only on P_n and P_E (L438)
   __device__ __forceinline__ void setup(const double (&Pn)[N], const double (&PE)[N], double dt_stage) {
-    idt = 1.0 / dt_stage;
-    itau = 1.0 / tau_;
+    idt = drcp(dt_stage);
+    itau = drcp(tau_);
     Pieces pn;
     full_state<N>(m, g, tau_, Pn, pn.th, pn.v, pn.b, pn.h);
     double Un[N];
     flux_vector<N>(g, 0, Pn, pn.th, pn.v, pn.b, pn.h, Un);
-    scale = sqrt(norm2sq<N>(Un)) * idt;
+    scale = dsqrt(norm2sq<N>(Un)) * idt;
     if constexpr (N == 10) {
       Thn = pn.th.Th;
 #pragma unroll
@@ -107,7 +107,7 @@ struct InvertProblem {
 
   __device__ __forceinline__ void setup() {
     double s2 = norm2sq<N>(Ustar);
-    iscale = 1.0 / sqrt(s2);
+    iscale = drcp(dsqrt(s2));
   }
   __device__ __forceinline__ void assemble(const double (&P)[N], const Pieces &pc, double (&R)[N]) const {
     double U[N];

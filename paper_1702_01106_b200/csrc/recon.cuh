@@ -4,6 +4,8 @@
 
 #include <math.h>
 
+#include "fp64ops.cuh"
+
 namespace grim {
 
 __device__ __forceinline__ double minmod2(double a, double b) {
@@ -32,7 +34,7 @@ __device__ __forceinline__ double limited_slope(double theta, double vm, double 
 // MP5 value at the i+1/2 face from v_{i-2..i+2}; alpha = 4, eps = 1e-10 (C-6)
 __device__ __forceinline__ double mp5_face(double vm2, double vm1, double v0, double vp1, double vp2) {
   const double alpha = 4.0, eps = 1e-10;
-  double vor = (2.0 * vm2 - 13.0 * vm1 + 47.0 * v0 + 27.0 * vp1 - 3.0 * vp2) / 60.0;
+  double vor = ddiv(2.0 * vm2 - 13.0 * vm1 + 47.0 * v0 + 27.0 * vp1 - 3.0 * vp2, 60.0);
   double vmp = v0 + minmod2(vp1 - v0, alpha * (v0 - vm1));
   if ((vor - v0) * (vor - vmp) <= eps) return vor;
   double dm1 = vm2 - 2.0 * vm1 + v0;
