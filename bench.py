@@ -27,7 +27,7 @@ METRIC = "fp64 zone-updates/sec per Newton step (EMHD 10-var) and % of HBM roofl
 UNIT = "zone-updates/s"
 
 # per zone and stage, Minkowski EMHD, 2 Newton iterations (measured with ncu, profiles/)
-ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 15000.0   # fp64-pipe thread instructions of the Newton kernel per zone
+ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 6114.0    # fp64-pipe thread instructions of the Newton kernel per zone (ncu, profiles/r1_ncu_full_stage_kernels.md)
 ALG_BYTES_PER_ZONE_STAGE_NEWTON = 8.0 * (10 + 10 + 10 + 10 + 3 + 10 + 1) + 4 * 4   # P^k,P_n,P_E,C,G in; P,|R| out; status,iters in/out
 FP64_INSTR_PER_CLK_PER_SM = 64.0                 # B200: 64 fp64 lanes per SM (guide: unit counts), 148 SMs
 N_SM = 148

@@ -181,6 +181,16 @@ int grim_get_geometry(grim_ctx *c, int32_t loc, int64_t idx2d, double *gcov, dou
  * on a full grid and returns fp64 instructions per second (host out).  Used for the ALU roofline denominator. */
 int grim_fp64_probe(grim_ctx *c, int32_t fma, int32_t iters, double *inst_per_s);
 
+/* Arithmetic self-test: the kernels form every fp64 quotient, reciprocal and square root
+ * speculatively as straight-line code that is IEEE-754 correctly rounded for operands of magnitude in
+ * [2^-480, 2^480), guarded by an exponent test, and replay a zone with the plain operators when a guard fails.
+ * This call compares the speculative operations with the plain operators bit for bit on n pseudo-random operand
+ * pairs on the device (wide = 0: exponents within +-400 of 1; wide = 1: the whole fp64 range with zeros, negative
+ * numbers, subnormals, infinities and NaNs, where the guard must reject what the straight-line code gets wrong).
+ * out6 (HOST): mismatches of [0] a/b, [1] 1/b, [2] sqrt(a), [3] a/60, [4] the zero-tolerant variants -- all must be
+ * 0 -- and [5] the number of a/b samples the guard accepted.  Synchronises. */
+int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t wide, int64_t *out6);
+
 /* End-to-end variants taking HOST buffers (pinned or pageable): copy in, run on the device, copy out, on the
  * context's stream; they return after the stream is synchronised.  Device staging buffers belong to the context.
  *   grim_timestep_host          : P_host N*Zg in/out; runs nsteps time steps (dt <= 0: chosen per step from cfl).

@@ -58,6 +58,7 @@ _SIGNATURES = {
     "grim_prim_to_conserved": (C.c_int, [_vp, _i64, _vp, _vp]),
     "grim_get_geometry": (C.c_int, [_vp, _i32, _i64, _pd, _pd, _pd, _pd, _pd, _pd]),
     "grim_fp64_probe": (C.c_int, [_vp, _i32, _i32, _pd]),
+    "grim_arith_selftest": (C.c_int, [_vp, _i64, _i64, _i32, _pi64]),
     "grim_timestep_host": (C.c_int, [_vp, _vp, _i32, _dbl, _pd]),
     "grim_invert_primitives_host": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp]),
     "grim_launch_count": (_i64, [_vp]),
@@ -280,3 +281,10 @@ class Grid:
         out = C.c_double(0.0)
         self._check(self._L.grim_fp64_probe(self.h, 1 if fma else 0, iters, C.byref(out)), "grim_fp64_probe")
         return out.value
+
+    def arith_selftest(self, n, seed=0, wide=False):
+        """-> (mismatches of [a/b, 1/b, sqrt, a/60, zero-tolerant variants], accepted a/b samples)"""
+        out = (C.c_int64 * 6)()
+        self._check(self._L.grim_arith_selftest(self.h, int(n), int(seed), 1 if wide else 0, out),
+                    "grim_arith_selftest")
+        return [int(x) for x in out[:5]], int(out[5])

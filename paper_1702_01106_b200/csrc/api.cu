@@ -528,6 +528,22 @@ extern "C" int grim_fp64_probe(grim_ctx *c, int32_t fma, int32_t iters, double *
   return check_launch(c, "fp64 probe");
 }
 
+extern "C" int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t wide, int64_t *out6) {
+  if (!c || !out6 || n < 0) return fail(c, GRIM_EINVAL, "grim_arith_selftest: bad argument");
+  CU(cudaSetDevice(c->d.device));
+  unsigned long long *d = nullptr;
+  CU(cudaMalloc((void **)&d, 6 * sizeof(unsigned long long)));
+  CU(cudaMemsetAsync(d, 0, 6 * sizeof(unsigned long long), c->stream));
+  c->launches += launch_arith_selftest((unsigned long long)n, (unsigned long long)seed, wide, d, c->stream);
+  unsigned long long h[6];
+  cudaError_t e = cudaMemcpyAsync(h, d, sizeof(h), cudaMemcpyDeviceToHost, c->stream);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+  cudaFree(d);
+  if (e != cudaSuccess) return fail(c, GRIM_ECUDA, cudaGetErrorString(e));
+  for (int k = 0; k < 6; k++) out6[k] = (int64_t)h[k];
+  return check_launch(c, "arith selftest");
+}
+
 extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used) {
   int rc = need_metric(c);
   if (rc) return rc;

@@ -101,6 +101,8 @@ int launch_metric_flat(const GridView &gv, double *geomC, double *geomF0, double
 int launch_stats(const GridView &gv, const double *Pn, double dt_stage, const double *resnorm,
                  const int32_t *status, const int32_t *iters, StatsDev *out, cudaStream_t s);
 int launch_copy_interior(const GridView &gv, const double *src, double *dst, cudaStream_t s);
+int launch_arith_selftest(unsigned long long n, unsigned long long seed, int wide, unsigned long long *out,
+                          cudaStream_t s);
 int launch_fp64_probe(int fma, int iters, double *sink, int blocks, int threads, cudaStream_t s);
 
 }  // namespace grim

@@ -16,21 +16,11 @@ namespace grim {
 
 static constexpr int FB = 128;
 
-template <int N, int RECON, class G, int DIR>  // DIR = 0..2
-__global__ void __launch_bounds__(FB)
-face_flux_kernel(GridView gv, const double *__restrict__ PE, double *__restrict__ Fface,
-                 double *__restrict__ cface) {
-  // faces: index range [ng, ng+n] along DIR, interior along the other directions
-  const int n0 = gv.n[0] + (DIR == 0), n1 = gv.n[1] + (DIR == 1), n2 = gv.n[2] + (DIR == 2);
-  const long long t = (long long)blockIdx.x * FB + threadIdx.x;
-  if (t >= (long long)n0 * n1 * n2) return;
-  const int i = (int)(t % n0) + gv.ngd[0];
-  const long long r = t / n0;
-  const int j = (int)(r % n1) + gv.ngd[1];
-  const int k = (int)(r / n1) + gv.ngd[2];
-  const long long z = zone_index(gv, i, j, k);
+// LLF flux and face speed of the lower DIR-face of padded zone z under arithmetic policy A
+template <int N, int RECON, class G, int DIR, class A>
+__device__ __forceinline__ void face_compute(A &ar, const GridView &gv, const double *__restrict__ PE, long long z,
+                                             int i, int j, double (&F)[N], double &c) {
   const long long stride = (DIR == 0) ? 1 : (DIR == 1) ? (long long)gv.sz[0] : (long long)gv.sz[0] * gv.sz[1];
-
   double Pm[N], Pp[N];  // P^- (from zone i-1) and P^+ (from zone i) at the face (L158-160)
 #pragma unroll
   for (int v = 0; v < N; v++) {
@@ -39,12 +29,12 @@ face_flux_kernel(GridView gv, const double *__restrict__ PE, double *__restrict_
     if constexpr (RECON == 1) {
       const double s0 = p[-3 * stride], s1 = p[-2 * stride], s2 = p[-stride], s3 = p[0], s4 = p[stride],
                    s5 = p[2 * stride];
-      hi = mp5_face(s0, s1, s2, s3, s4);
-      lo = mp5_face(s5, s4, s3, s2, s1);
+      hi = mp5_face(ar, s0, s1, s2, s3, s4);
+      lo = mp5_face(ar, s5, s4, s3, s2, s1);
     } else {
       const double s1 = p[-2 * stride], s2 = p[-stride], s3 = p[0], s4 = p[stride];
-      reconstruct<0>(gv.theta, 0.0, s1, s2, s3, 0.0, hi, unused);
-      reconstruct<0>(gv.theta, 0.0, s2, s3, s4, 0.0, unused, lo);
+      reconstruct<0>(ar, gv.theta, 0.0, s1, s2, s3, 0.0, hi, unused);
+      reconstruct<0>(ar, gv.theta, 0.0, s2, s3, s4, 0.0, unused, lo);
     }
     Pm[v] = hi;
     Pp[v] = lo;
@@ -55,30 +45,254 @@ face_flux_kernel(GridView gv, const double *__restrict__ PE, double *__restrict_
   if constexpr (!G::flat) load_geom<DIR + 1>(gv.geomF[DIR], gv.n2d, (long long)j * gv.sz[0] + i, g, tau);
 
   Pieces sm, sp;
-  full_state<N>(gv.m, g, tau, Pm, sm.th, sm.v, sm.b, sm.h);
-  full_state<N>(gv.m, g, tau, Pp, sp.th, sp.v, sp.b, sp.h);
+  full_state<N>(ar, gv.m, g, tau, Pm, sm.th, sm.v, sm.b, sm.h);
+  full_state<N>(ar, gv.m, g, tau, Pp, sp.th, sp.v, sp.b, sp.h);
   double Um[N], Up[N], Fm[N], Fp[N];
   flux_vector<N>(g, 0, Pm, sm.th, sm.v, sm.b, sm.h, Um);
   flux_vector<N>(g, 0, Pp, sp.th, sp.v, sp.b, sp.h, Up);
   flux_vector<N>(g, DIR + 1, Pm, sm.th, sm.v, sm.b, sm.h, Fm);
   flux_vector<N>(g, DIR + 1, Pp, sp.th, sp.v, sp.b, sp.h, Fp);
-  const double cm = cmax_dir(g, vmax2<N>(gv.m, tau, Pm[RHO], Pm[UU], sm.b.bsq), sm.v.ucon[0], sm.v.ucon[DIR + 1]);
-  const double cp = cmax_dir(g, vmax2<N>(gv.m, tau, Pp[RHO], Pp[UU], sp.b.bsq), sp.v.ucon[0], sp.v.ucon[DIR + 1]);
-  const double c = fmax(cm, cp);  // L164: c_max >= max |c^+-| over both states
+  const double cm =
+      cmax_dir(ar, g, vmax2<N>(ar, gv.m, tau, Pm[RHO], Pm[UU], sm.b.bsq), sm.v.ucon[0], sm.v.ucon[DIR + 1]);
+  const double cp =
+      cmax_dir(ar, g, vmax2<N>(ar, gv.m, tau, Pp[RHO], Pp[UU], sp.b.bsq), sp.v.ucon[0], sp.v.ucon[DIR + 1]);
+  c = fmax(cm, cp);  // L164: c_max >= max |c^+-| over both states
 #pragma unroll
-  for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = 0.5 * (Fp[v] + Fm[v]) - 0.5 * c * (Up[v] - Um[v]);  // eq 17
+  for (int v = 0; v < N; v++) F[v] = 0.5 * (Fp[v] + Fm[v]) - 0.5 * c * (Up[v] - Um[v]);  // eq 17
+}
+
+template <int N, int RECON, class G, int DIR>
+__device__ __noinline__ void face_replay(const GridView &gv, const double *__restrict__ PE, long long z, int i, int j,
+                                         double *__restrict__ Fface, double *__restrict__ cface) {
+  ExactArith ar;
+  double F[N], c;
+  face_compute<N, RECON, G, DIR>(ar, gv, PE, z, i, j, F, c);
+#pragma unroll
+  for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
   cface[z] = c;
+}
+
+#ifndef GRIM_FLUX_MINB
+#define GRIM_FLUX_MINB 4
+#endif
+template <int N, int RECON, class G, int DIR>  // DIR = 0..2
+__global__ void __launch_bounds__(FB, GRIM_FLUX_MINB)
+face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE, double *__restrict__ Fface,
+                 double *__restrict__ cface) {
+  // faces: index range [ng, ng+n] along DIR, interior along the other directions
+  const int n0 = gv.n[0] + (DIR == 0), n1 = gv.n[1] + (DIR == 1), n2 = gv.n[2] + (DIR == 2);
+  const long long t = (long long)blockIdx.x * FB + threadIdx.x;
+  if (t >= (long long)n0 * n1 * n2) return;
+  const int i = (int)(t % n0) + gv.ngd[0];
+  const long long r = t / n0;
+  const int j = (int)(r % n1) + gv.ngd[1];
+  const int k = (int)(r / n1) + gv.ngd[2];
+  const long long z = zone_index(gv, i, j, k);
+  SpecArith ar;
+  double F[N], c;
+  face_compute<N, RECON, G, DIR>(ar, gv, PE, z, i, j, F, c);
+  if (ar.good()) {
+#pragma unroll
+    for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
+    cface[z] = c;
+  } else {
+    face_replay<N, RECON, G, DIR>(gv, PE, z, i, j, Fface, cface);
+  }
 }
 
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, double v) {
   atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
 
+// Stage constant, EMHD gradient terms and wave-speed figures of padded zone z under arithmetic policy A
+template <int N, class G, class A>
+__device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, const double *__restrict__ PE,
+                                                    const double *__restrict__ Pn, double dt_stage,
+                                                    const double *__restrict__ Fface,
+                                                    const double *__restrict__ cface, long long z, long long id,
+                                                    double (&Cout)[N], double (&Gout)[3], double (&sp_loc)[4]) {
+  const double idt = ar.rcp(dt_stage);
+  G gc;
+  double tau = gv.tau_const;
+  if constexpr (!G::flat) load_geom<0>(gv.geomC, gv.n2d, id, gc, tau);
+
+  double Pn_z[N], PE_z[N];
+#pragma unroll
+  for (int v = 0; v < N; v++) {
+    Pn_z[v] = Pn[v * gv.zg + z];
+    PE_z[v] = PE[v * gv.zg + z];
+  }
+  Pieces sn, sE;
+  full_state<N>(ar, gv.m, gc, tau, Pn_z, sn.th, sn.v, sn.b, sn.h);
+  full_state<N>(ar, gv.m, gc, tau, PE_z, sE.th, sE.v, sE.b, sE.h);
+  double Un[N];
+  flux_vector<N>(gc, 0, Pn_z, sn.th, sn.v, sn.b, sn.h, Un);
+
+  // flux divergence (eq 10) and wave-speed figures (C-15)
+  double divF[N];
+#pragma unroll
+  for (int v = 0; v < N; v++) divF[v] = 0.0;
+  double ssum = 0.0;
+  const long long strides[3] = {1, (long long)gv.sz[0], (long long)gv.sz[0] * gv.sz[1]};
+#pragma unroll
+  for (int a = 0; a < 3; a++) {
+    if (gv.ngd[a] == 0) continue;
+    const double *Fa = Fface + (long long)a * N * gv.zg;
+    const double *ca = cface + (long long)a * gv.zg;
+    const long long zu = z + strides[a];
+#pragma unroll
+    for (int v = 0; v < N; v++) divF[v] = divF[v] + (Fa[v * gv.zg + zu] - Fa[v * gv.zg + z]) * gv.idx[a];
+    const double cz = fmax(ca[z], ca[zu]) * gv.idx[a];
+    sp_loc[a] = cz;
+    ssum = ssum + cz;
+  }
+  sp_loc[3] = ssum;
+
+  // explicit geometric source sqrt(-g) T^k_l Gamma^l_{nu k} at P_E (eq 31; C-5)
+  double SE[4] = {0.0, 0.0, 0.0, 0.0};
+  if constexpr (!G::flat) {
+    double T[4][4];
+    double q = 0.0, dP = 0.0;
+    if constexpr (N == 10) { q = PE_z[QQ]; dP = PE_z[DPP]; }
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) stress_row<N>(mu, PE_z[RHO], PE_z[UU], q, dP, sE.th, sE.v, sE.b, sE.h, T[mu]);
+#pragma unroll
+    for (int nu = 0; nu < 4; nu++) {
+      double s = 0.0;
+#pragma unroll
+      for (int kk = 0; kk < 4; kk++)
+#pragma unroll
+        for (int l = 0; l < 4; l++) s = s + T[kk][l] * gv.conn[(l * 16 + nu * 4 + kk) * gv.n2d + id];
+      SE[nu] = gc.sqrtmg() * s;
+    }
+  }
+#pragma unroll
+  for (int v = 0; v < N; v++) {
+    double c = -Un[v] * idt + divF[v];
+    if constexpr (!G::flat) {
+      if (v >= 1 && v <= 4) c = c - SE[v - 1];
+    }
+    Cout[v] = c;
+  }
+
+  // spatial-gradient parts of the EMHD sources: limited 3-point slopes of derived quantities (L115; O-8)
+  if constexpr (N == 10) {
+    double dTheta[4] = {0.0, 0.0, 0.0, 0.0};
+    double ducov[4][4];
+#pragma unroll
+    for (int a = 0; a < 4; a++)
+#pragma unroll
+      for (int b = 0; b < 4; b++) ducov[a][b] = 0.0;
+    double divx = 0.0;
+    const double th = gv.theta;
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      if (gv.ngd[a] == 0) continue;
+      const long long zm = z - strides[a], zp = z + strides[a];
+      double Pm_[N], Pp_[N];
+#pragma unroll
+      for (int v = 0; v < N; v++) {
+        Pm_[v] = PE[v * gv.zg + zm];
+        Pp_[v] = PE[v * gv.zg + zp];
+      }
+      G gm, gp;
+      double taum = tau, taup = tau;
+      double sgm = 1.0, sgp = 1.0, sgc = 1.0;
+      if constexpr (!G::flat) {
+        const long long idm = (a == 0) ? id - 1 : (a == 1) ? id - gv.sz[0] : id;
+        const long long idp = (a == 0) ? id + 1 : (a == 1) ? id + gv.sz[0] : id;
+        load_geom<0>(gv.geomC, gv.n2d, idm, gm, taum);
+        load_geom<0>(gv.geomC, gv.n2d, idp, gp, taup);
+        sgm = gm.sg; sgp = gp.sg; sgc = gc.sg;
+      }
+      Vel vm_, vp_;
+      vel_state(ar, gm, Pm_[U1], Pm_[U2], Pm_[U3], vm_);
+      vel_state(ar, gp, Pp_[U1], Pp_[U2], Pp_[U3], vp_);
+      const double Thm = ar.div(gv.m.gm1 * Pm_[UU], Pm_[RHO]);
+      const double Thp = ar.div(gv.m.gm1 * Pp_[UU], Pp_[RHO]);
+      dTheta[a + 1] = limited_slope(th, Thm, sE.th.Th, Thp) * gv.idx[a];
+#pragma unroll
+      for (int nu = 0; nu < 4; nu++)
+        ducov[a + 1][nu] = limited_slope(th, vm_.ucov[nu], sE.v.ucov[nu], vp_.ucov[nu]) * gv.idx[a];
+      if constexpr (G::flat) {
+        divx = divx + limited_slope(th, vm_.ucon[a + 1], sE.v.ucon[a + 1], vp_.ucon[a + 1]) * gv.idx[a];
+      } else {
+        divx = divx + limited_slope(th, sgm * vm_.ucon[a + 1], sgc * sE.v.ucon[a + 1], sgp * vp_.ucon[a + 1]) *
+                          gv.idx[a];
+      }
+    }
+    if constexpr (!G::flat) divx = ar.div_z(divx, gc.sqrtmg());
+    // Xq = bhat^i d_i Theta + Theta bhat^mu (u^i d_i u_mu - Gamma^l_{nu mu} u^nu u_l)
+    // Xd = bhat^i bhat^nu d_i u_nu - Gamma^l_{mu nu} bhat^mu bhat^nu u_l
+    const double *bh = sE.h.con;
+    const double *ucon = sE.v.ucon, *ucov = sE.v.ucov;
+    double bgradTh = bh[1] * dTheta[1];
+    bgradTh = bgradTh + bh[2] * dTheta[2];
+    bgradTh = bgradTh + bh[3] * dTheta[3];
+    double ba = 0.0;
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) {
+      double acc = ucon[1] * ducov[1][mu];
+      acc = acc + ucon[2] * ducov[2][mu];
+      acc = acc + ucon[3] * ducov[3][mu];
+      if constexpr (!G::flat) {
+        double gam = 0.0;
+#pragma unroll
+        for (int nu = 0; nu < 4; nu++)
+#pragma unroll
+          for (int l = 0; l < 4; l++)
+            gam = gam + gv.conn[(l * 16 + nu * 4 + mu) * gv.n2d + id] * ucon[nu] * ucov[l];
+        acc = acc - gam;
+      }
+      ba = ba + bh[mu] * acc;
+    }
+    double bbdu = 0.0;
+#pragma unroll
+    for (int ii = 1; ii < 4; ii++) {
+      double s = bh[0] * ducov[ii][0];
+      s = s + bh[1] * ducov[ii][1];
+      s = s + bh[2] * ducov[ii][2];
+      s = s + bh[3] * ducov[ii][3];
+      bbdu = bbdu + bh[ii] * s;
+    }
+    double Xd = bbdu;
+    if constexpr (!G::flat) {
+      double gbb = 0.0;
+#pragma unroll
+      for (int mu = 0; mu < 4; mu++)
+#pragma unroll
+        for (int nu = 0; nu < 4; nu++)
+#pragma unroll
+          for (int l = 0; l < 4; l++)
+            gbb = gbb + gv.conn[(l * 16 + mu * 4 + nu) * gv.n2d + id] * bh[mu] * bh[nu] * ucov[l];
+      Xd = bbdu - gbb;
+    }
+    Gout[0] = bgradTh + sE.th.Th * ba;
+    Gout[1] = Xd;
+    Gout[2] = divx;
+  }
+}
+
 template <int N, class G>
-__global__ void __launch_bounds__(FB)
-stage_const_kernel(GridView gv, const double *__restrict__ PE, const double *__restrict__ Pn, double dt_stage,
-                   const double *__restrict__ Fface, const double *__restrict__ cface, double *__restrict__ C,
-                   double *__restrict__ Gx, Counters *cnt) {
+__device__ __noinline__ void stage_const_replay(const GridView &gv, const double *__restrict__ PE,
+                                                const double *__restrict__ Pn, double dt_stage,
+                                                const double *__restrict__ Fface, const double *__restrict__ cface,
+                                                long long z, long long id, double *Cout, double *Gout,
+                                                double *sp_loc) {
+  ExactArith ar;
+  double C_[N], G_[3] = {0.0, 0.0, 0.0}, s_[4] = {0.0, 0.0, 0.0, 0.0};
+  stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, z, id, C_, G_, s_);
+  for (int v = 0; v < N; v++) Cout[v] = C_[v];
+  for (int v = 0; v < 3; v++) Gout[v] = G_[v];
+  for (int v = 0; v < 4; v++) sp_loc[v] = s_[v];
+}
+
+template <int N, class G>
+__global__ void __launch_bounds__(FB, 4)
+stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE,
+                   const double *__restrict__ Pn, double dt_stage, const double *__restrict__ Fface,
+                   const double *__restrict__ cface, double *__restrict__ C, double *__restrict__ Gx,
+                   Counters *cnt) {
   const long long t = (long long)blockIdx.x * FB + threadIdx.x;
   double sp_loc[4] = {0.0, 0.0, 0.0, 0.0};
   if (t < gv.nint) {
@@ -86,165 +300,15 @@ stage_const_kernel(GridView gv, const double *__restrict__ PE, const double *__r
     zone_coords(gv, t, i, j, k);
     const long long z = zone_index(gv, i, j, k);
     const long long id = (long long)j * gv.sz[0] + i;
-    const double idt = drcp(dt_stage);
-    G gc;
-    double tau = gv.tau_const;
-    if constexpr (!G::flat) load_geom<0>(gv.geomC, gv.n2d, id, gc, tau);
-
-    double Pn_z[N], PE_z[N];
+    double Cout[N], Gout[3] = {0.0, 0.0, 0.0};
+    SpecArith ar;
+    stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, z, id, Cout, Gout, sp_loc);
+    if (!ar.good()) stage_const_replay<N, G>(gv, PE, Pn, dt_stage, Fface, cface, z, id, Cout, Gout, sp_loc);
 #pragma unroll
-    for (int v = 0; v < N; v++) {
-      Pn_z[v] = Pn[v * gv.zg + z];
-      PE_z[v] = PE[v * gv.zg + z];
-    }
-    Pieces sn, sE;
-    full_state<N>(gv.m, gc, tau, Pn_z, sn.th, sn.v, sn.b, sn.h);
-    full_state<N>(gv.m, gc, tau, PE_z, sE.th, sE.v, sE.b, sE.h);
-    double Un[N];
-    flux_vector<N>(gc, 0, Pn_z, sn.th, sn.v, sn.b, sn.h, Un);
-
-    // flux divergence (eq 10) and wave-speed figures (C-15)
-    double divF[N];
-#pragma unroll
-    for (int v = 0; v < N; v++) divF[v] = 0.0;
-    double ssum = 0.0;
-    const long long strides[3] = {1, (long long)gv.sz[0], (long long)gv.sz[0] * gv.sz[1]};
-#pragma unroll
-    for (int a = 0; a < 3; a++) {
-      if (gv.ngd[a] == 0) continue;
-      const double *Fa = Fface + (long long)a * N * gv.zg;
-      const double *ca = cface + (long long)a * gv.zg;
-      const long long zu = z + strides[a];
-#pragma unroll
-      for (int v = 0; v < N; v++) divF[v] = divF[v] + (Fa[v * gv.zg + zu] - Fa[v * gv.zg + z]) * gv.idx[a];
-      const double cz = fmax(ca[z], ca[zu]) * gv.idx[a];
-      sp_loc[a] = cz;
-      ssum = ssum + cz;
-    }
-    sp_loc[3] = ssum;
-
-    // explicit geometric source sqrt(-g) T^k_l Gamma^l_{nu k} at P_E (eq 31; C-5)
-    double SE[4] = {0.0, 0.0, 0.0, 0.0};
-    if constexpr (!G::flat) {
-      double T[4][4];
-      double q = 0.0, dP = 0.0;
-      if constexpr (N == 10) { q = PE_z[QQ]; dP = PE_z[DPP]; }
-#pragma unroll
-      for (int mu = 0; mu < 4; mu++) stress_row<N>(mu, PE_z[RHO], PE_z[UU], q, dP, sE.th, sE.v, sE.b, sE.h, T[mu]);
-#pragma unroll
-      for (int nu = 0; nu < 4; nu++) {
-        double s = 0.0;
-#pragma unroll
-        for (int kk = 0; kk < 4; kk++)
-#pragma unroll
-          for (int l = 0; l < 4; l++) s = s + T[kk][l] * gv.conn[(l * 16 + nu * 4 + kk) * gv.n2d + id];
-        SE[nu] = gc.sqrtmg() * s;
-      }
-    }
-#pragma unroll
-    for (int v = 0; v < N; v++) {
-      double c = -Un[v] * idt + divF[v];
-      if constexpr (!G::flat) {
-        if (v >= 1 && v <= 4) c = c - SE[v - 1];
-      }
-      C[v * gv.zg + z] = c;
-    }
-
-    // spatial-gradient parts of the EMHD sources: limited 3-point slopes of derived quantities (L115; O-8)
+    for (int v = 0; v < N; v++) C[v * gv.zg + z] = Cout[v];
     if constexpr (N == 10) {
-      double dTheta[4] = {0.0, 0.0, 0.0, 0.0};
-      double ducov[4][4];
 #pragma unroll
-      for (int a = 0; a < 4; a++)
-#pragma unroll
-        for (int b = 0; b < 4; b++) ducov[a][b] = 0.0;
-      double divx = 0.0;
-      const double th = gv.theta;
-#pragma unroll
-      for (int a = 0; a < 3; a++) {
-        if (gv.ngd[a] == 0) continue;
-        const long long zm = z - strides[a], zp = z + strides[a];
-        double Pm_[N], Pp_[N];
-#pragma unroll
-        for (int v = 0; v < N; v++) {
-          Pm_[v] = PE[v * gv.zg + zm];
-          Pp_[v] = PE[v * gv.zg + zp];
-        }
-        G gm, gp;
-        double taum = tau, taup = tau;
-        double sgm = 1.0, sgp = 1.0, sgc = 1.0;
-        if constexpr (!G::flat) {
-          const long long idm = (a == 0) ? id - 1 : (a == 1) ? id - gv.sz[0] : id;
-          const long long idp = (a == 0) ? id + 1 : (a == 1) ? id + gv.sz[0] : id;
-          load_geom<0>(gv.geomC, gv.n2d, idm, gm, taum);
-          load_geom<0>(gv.geomC, gv.n2d, idp, gp, taup);
-          sgm = gm.sg; sgp = gp.sg; sgc = gc.sg;
-        }
-        Vel vm_, vp_;
-        vel_state(gm, Pm_[U1], Pm_[U2], Pm_[U3], vm_);
-        vel_state(gp, Pp_[U1], Pp_[U2], Pp_[U3], vp_);
-        const double Thm = ddiv(gv.m.gm1 * Pm_[UU], Pm_[RHO]);
-        const double Thp = ddiv(gv.m.gm1 * Pp_[UU], Pp_[RHO]);
-        dTheta[a + 1] = limited_slope(th, Thm, sE.th.Th, Thp) * gv.idx[a];
-#pragma unroll
-        for (int nu = 0; nu < 4; nu++)
-          ducov[a + 1][nu] = limited_slope(th, vm_.ucov[nu], sE.v.ucov[nu], vp_.ucov[nu]) * gv.idx[a];
-        if constexpr (G::flat) {
-          divx = divx + limited_slope(th, vm_.ucon[a + 1], sE.v.ucon[a + 1], vp_.ucon[a + 1]) * gv.idx[a];
-        } else {
-          divx = divx + limited_slope(th, sgm * vm_.ucon[a + 1], sgc * sE.v.ucon[a + 1], sgp * vp_.ucon[a + 1]) *
-                            gv.idx[a];
-        }
-      }
-      if constexpr (!G::flat) divx = ddiv(divx, gc.sqrtmg());
-      // Xq = bhat^i d_i Theta + Theta bhat^mu (u^i d_i u_mu - Gamma^l_{nu mu} u^nu u_l)
-      // Xd = bhat^i bhat^nu d_i u_nu - Gamma^l_{mu nu} bhat^mu bhat^nu u_l
-      const double *bh = sE.h.con;
-      const double *ucon = sE.v.ucon, *ucov = sE.v.ucov;
-      double bgradTh = bh[1] * dTheta[1];
-      bgradTh = bgradTh + bh[2] * dTheta[2];
-      bgradTh = bgradTh + bh[3] * dTheta[3];
-      double ba = 0.0;
-#pragma unroll
-      for (int mu = 0; mu < 4; mu++) {
-        double acc = ucon[1] * ducov[1][mu];
-        acc = acc + ucon[2] * ducov[2][mu];
-        acc = acc + ucon[3] * ducov[3][mu];
-        if constexpr (!G::flat) {
-          double gam = 0.0;
-#pragma unroll
-          for (int nu = 0; nu < 4; nu++)
-#pragma unroll
-            for (int l = 0; l < 4; l++)
-              gam = gam + gv.conn[(l * 16 + nu * 4 + mu) * gv.n2d + id] * ucon[nu] * ucov[l];
-          acc = acc - gam;
-        }
-        ba = ba + bh[mu] * acc;
-      }
-      double bbdu = 0.0;
-#pragma unroll
-      for (int ii = 1; ii < 4; ii++) {
-        double s = bh[0] * ducov[ii][0];
-        s = s + bh[1] * ducov[ii][1];
-        s = s + bh[2] * ducov[ii][2];
-        s = s + bh[3] * ducov[ii][3];
-        bbdu = bbdu + bh[ii] * s;
-      }
-      double Xd = bbdu;
-      if constexpr (!G::flat) {
-        double gbb = 0.0;
-#pragma unroll
-        for (int mu = 0; mu < 4; mu++)
-#pragma unroll
-          for (int nu = 0; nu < 4; nu++)
-#pragma unroll
-            for (int l = 0; l < 4; l++)
-              gbb = gbb + gv.conn[(l * 16 + mu * 4 + nu) * gv.n2d + id] * bh[mu] * bh[nu] * ucov[l];
-        Xd = bbdu - gbb;
-      }
-      Gx[0 * gv.zg + z] = bgradTh + sE.th.Th * ba;
-      Gx[1 * gv.zg + z] = Xd;
-      Gx[2 * gv.zg + z] = divx;
+      for (int v = 0; v < 3; v++) Gx[v * gv.zg + z] = Gout[v];
     }
   }
   // block max of the wave-speed figures -> global atomic max

@@ -256,7 +256,8 @@ __global__ void stats_kernel(GridView gv, const double *__restrict__ Pn, double 
 #pragma unroll
   for (int v = 0; v < N; v++) P[v] = Pn[v * gv.zg + z];
   Pieces pc;
-  full_state<N>(gv.m, g, tau, P, pc.th, pc.v, pc.b, pc.h);
+  ExactArith ar;
+  full_state<N>(ar, gv.m, g, tau, P, pc.th, pc.v, pc.b, pc.h);
   flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
   const double sc = sqrt(norm2sq<N>(U)) / dt_stage;
   const double rel = resnorm[z] / sc;
@@ -315,6 +316,90 @@ __global__ void fp64_probe_kernel(int iters, double *sink) {
   }
   const double s = a0 + a1 + a2 + a3 + a4 + a5 + a6 + a7;
   if (s == 123.456) sink[0] = s;
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// Arithmetic self-test: SpecArith against ExactArith (the IEEE operators), operation by operation, on
+// pseudo-random operands.  Sample n of a launch: two 64-bit hashes (splitmix64 of the counter) give the
+// mantissas; exponents cycle through the whole fp64 range in `wide` mode (the in-range guard must then reject
+// what the straight-line code gets wrong) or stay within +-400 of 1.  A sample counts as a mismatch when the
+// speculative result differs in any bit from the exact one while the policy still reports ok.
+// out[0..4]: mismatches of div, rcp, sqrt, div60, div_z/sqrt_z; out[5]: samples the guard accepted.
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long splitmix64(unsigned long long x) {
+  x += 0x9E3779B97F4A7C15ULL;
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ULL;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBULL;
+  return x ^ (x >> 31);
+}
+__device__ __forceinline__ bool same_bits(double a, double b) {
+  return __double_as_longlong(a) == __double_as_longlong(b) || (a != a && b != b);
+}
+__global__ void arith_selftest_kernel(unsigned long long n, unsigned long long seed, int wide,
+                                      unsigned long long *out) {
+  unsigned long long bad[5] = {0, 0, 0, 0, 0}, accepted = 0;
+  for (unsigned long long t = (unsigned long long)blockIdx.x * blockDim.x + threadIdx.x; t < n;
+       t += (unsigned long long)gridDim.x * blockDim.x) {
+    const unsigned long long h1 = splitmix64(seed + 2 * t), h2 = splitmix64(seed + 2 * t + 1);
+    unsigned long long ma = h1 & 0x000FFFFFFFFFFFFFULL, mb = h2 & 0x000FFFFFFFFFFFFFULL;
+    // every 8th sample: mantissas at the ends of the binade (all zeros / all ones / one bit), the hard cases
+    if ((t & 7) == 7) {
+      const unsigned sel = (unsigned)(h1 >> 52) & 3;
+      ma = sel == 0 ? 0 : sel == 1 ? 0x000FFFFFFFFFFFFFULL : sel == 2 ? (1ULL << ((h1 >> 54) % 52)) : ma;
+      const unsigned sel2 = (unsigned)(h2 >> 52) & 3;
+      mb = sel2 == 0 ? 0 : sel2 == 1 ? 0x000FFFFFFFFFFFFFULL : sel2 == 2 ? (0x000FFFFFFFFFFFFFULL ^ (1ULL << ((h2 >> 54) % 52))) : mb;
+    }
+    unsigned long long ea, eb;
+    if (wide) {
+      ea = (h1 >> 52) & 0x7FF;
+      eb = (h2 >> 52) & 0x7FF;
+    } else {
+      ea = 1023 - 400 + ((h1 >> 52) & 0x7FF) % 801;
+      eb = 1023 - 400 + ((h2 >> 52) & 0x7FF) % 801;
+    }
+    const unsigned long long sa = wide ? (h1 >> 63) << 63 : 0, sb = (h2 >> 63) << 63;
+    const double a = __longlong_as_double((long long)(sa | (ea << 52) | ma));
+    const double b = __longlong_as_double((long long)(sb | (eb << 52) | mb));
+    const double az = ((t & 63) == 5) ? (wide && (t & 64) ? -0.0 : 0.0) : a;
+    ExactArith ex;
+    {
+      SpecArith sp;
+      const double r = sp.div(a, b);
+      if (sp.ok) { accepted++; if (!same_bits(r, ex.div(a, b))) bad[0]++; }
+    }
+    {
+      SpecArith sp;
+      const double r = sp.rcp(b);
+      if (sp.ok && !same_bits(r, ex.rcp(b))) bad[1]++;
+    }
+    {
+      SpecArith sp;
+      const double r = sp.sqrt(a);
+      if (sp.ok && !same_bits(r, ex.sqrt(a))) bad[2]++;
+    }
+    {
+      SpecArith sp;
+      const double r = div60(sp, az);
+      if (sp.ok && !same_bits(r, div60(ex, az))) bad[3]++;
+    }
+    {
+      SpecArith sp;
+      const double r = sp.div_z(az, b);
+      if (sp.ok && !same_bits(r, ex.div_z(az, b))) bad[4]++;
+      SpecArith sq;
+      const double r2 = sq.sqrt_z(az);
+      if (sq.ok && !same_bits(r2, ex.sqrt_z(az))) bad[4]++;
+    }
+  }
+  for (int k = 0; k < 5; k++)
+    if (bad[k]) atomicAdd(&out[k], bad[k]);
+  if (accepted) atomicAdd(&out[5], accepted);
+}
+
+int launch_arith_selftest(unsigned long long n, unsigned long long seed, int wide, unsigned long long *out,
+                          cudaStream_t s) {
+  arith_selftest_kernel<<<148 * 8, 256, 0, s>>>(n, seed, wide, out);
+  return 1;
 }
 
 int launch_fp64_probe(int fma, int iters, double *sink, int blocks, int threads, cudaStream_t s) {

@@ -9,63 +9,88 @@ namespace grim {
 
 static constexpr int NB = 128;  // threads per block; 2 blocks/SM: 2 x 128 x (N*N*8 B) of Jacobian + 255 registers
 
+struct StageArgs {
+  const double *Pn, *PE, *C, *Gx;
+  double dt_stage;
+  int max_iters;
+  double *Piter, *resnorm;
+  int32_t *status, *iters;
+};
+
+// One zone of one stage under arithmetic policy A: loads, set-up, Newton iteration, stores.  Returns false
+// WITHOUT storing when a speculative operation saw an operand outside its safe range (fp64ops.cuh); the caller
+// then replays the zone with ExactArith.  Otherwise packs (rejected line-search trials << 1) | still-active.
+template <int N, class G, class A>
+__device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const StageArgs &a, long long z, int i, int j,
+                                          int st, double *sj) {
+  StageProblem<N, G> prob;
+  prob.m = gv.m;
+  if constexpr (G::flat) {
+    prob.tau_ = gv.tau_const;
+  } else {
+    load_geom<0>(gv.geomC, gv.n2d, (long long)j * gv.sz[0] + i, prob.g, prob.tau_);
+  }
+  double P[N];
+  {
+    double Pn_z[N], PE_z[N];
+#pragma unroll
+    for (int v = 0; v < N; v++) {
+      Pn_z[v] = a.Pn[v * gv.zg + z];
+      PE_z[v] = a.PE[v * gv.zg + z];
+      P[v] = a.Piter[v * gv.zg + z];
+      prob.C[v] = a.C[v * gv.zg + z];
+    }
+    if constexpr (N == 10) {
+      prob.Xq = a.Gx[0 * gv.zg + z];
+      prob.Xd = a.Gx[1 * gv.zg + z];
+      prob.divx = a.Gx[2 * gv.zg + z];
+    }
+    prob.setup(ar, Pn_z, PE_z, a.dt_stage);
+  }
+  const double tol = gv.sp.atol + gv.sp.rtol * prob.scale;
+  int it = a.iters[z];
+  int nbt = 0;
+  JacView<N, NB> jac{sj};
+  double rn = newton_zone<N, NB>(ar, prob, gv.sp, tol, P, it, st, a.max_iters, jac, nbt);
+  if (!ar.good()) return -1;
+#pragma unroll
+  for (int v = 0; v < N; v++) a.Piter[v * gv.zg + z] = P[v];
+  a.resnorm[z] = rn;
+  a.status[z] = st;
+  a.iters[z] = it;
+  return (nbt << 1) | ((st & ST_TERMINAL) ? 0 : 1);
+}
+
+template <int N, class G>
+__device__ __noinline__ int stage_zone_replay(const GridView &gv, const StageArgs &a, long long z, int i, int j,
+                                              int st, double *sj) {
+  ExactArith ar;
+  return stage_zone<N, G>(ar, gv, a, z, i, j, st, sj);
+}
+
 template <int N, class G>
 __global__ void __launch_bounds__(NB, 2)
-newton_stage_kernel(GridView gv, const double *__restrict__ Pn, const double *__restrict__ PE,
-                    const double *__restrict__ C, const double *__restrict__ Gx, double dt_stage, int max_iters,
-                    double *__restrict__ Piter, double *__restrict__ resnorm, int32_t *__restrict__ status,
-                    int32_t *__restrict__ iters, Counters *cnt) {
+newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
-  int nbt = 0, active_after = 0;
+  int res = 0;
   if (t < gv.nint) {
     int i, j, k;
     zone_coords(gv, t, i, j, k);
     const long long z = zone_index(gv, i, j, k);
-    int st = status[z];
+    const int st = a.status[z];
     if (!(st & ST_TERMINAL)) {
-      StageProblem<N, G> prob;
-      prob.m = gv.m;
-      if constexpr (G::flat) {
-        prob.tau_ = gv.tau_const;
-      } else {
-        load_geom<0>(gv.geomC, gv.n2d, (long long)j * gv.sz[0] + i, prob.g, prob.tau_);
-      }
-      double P[N];
-      {
-        double Pn_z[N], PE_z[N];
-#pragma unroll
-        for (int v = 0; v < N; v++) {
-          Pn_z[v] = Pn[v * gv.zg + z];
-          PE_z[v] = PE[v * gv.zg + z];
-          P[v] = Piter[v * gv.zg + z];
-          prob.C[v] = C[v * gv.zg + z];
-        }
-        if constexpr (N == 10) {
-          prob.Xq = Gx[0 * gv.zg + z];
-          prob.Xd = Gx[1 * gv.zg + z];
-          prob.divx = Gx[2 * gv.zg + z];
-        }
-        prob.setup(Pn_z, PE_z, dt_stage);
-      }
-      const double tol = gv.sp.atol + gv.sp.rtol * prob.scale;
-      int it = iters[z];
-      JacView<N, NB> jac{smem + threadIdx.x};
-      double rn = newton_zone<N, NB>(prob, gv.sp, tol, P, it, st, max_iters, jac, nbt);
-#pragma unroll
-      for (int v = 0; v < N; v++) Piter[v * gv.zg + z] = P[v];
-      resnorm[z] = rn;
-      status[z] = st;
-      iters[z] = it;
-      active_after = (st & ST_TERMINAL) ? 0 : 1;
+      SpecArith ar;
+      res = stage_zone<N, G>(ar, gv, a, z, i, j, st, smem + threadIdx.x);
+      if (res < 0) res = stage_zone_replay<N, G>(gv, a, z, i, j, st, smem + threadIdx.x);
     }
   }
   // warp-aggregated counters
-  unsigned long long a = __reduce_add_sync(0xffffffffu, (unsigned)active_after);
-  unsigned long long b = __reduce_add_sync(0xffffffffu, (unsigned)nbt);
+  unsigned long long na = __reduce_add_sync(0xffffffffu, (unsigned)(res & 1));
+  unsigned long long nb = __reduce_add_sync(0xffffffffu, (unsigned)(res >> 1));
   if ((threadIdx.x & 31) == 0) {
-    if (a) atomicAdd(&cnt->n_active, a);
-    if (b) atomicAdd(&cnt->backtracks, b);
+    if (na) atomicAdd(&cnt->n_active, na);
+    if (nb) atomicAdd(&cnt->backtracks, nb);
   }
 }
 
@@ -80,8 +105,8 @@ static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE
     attr_set = true;
   }
   const long long blocks = (gv.nint + NB - 1) / NB;
-  newton_stage_kernel<N, G><<<(unsigned)blocks, NB, smem, s>>>(gv, Pn, PE, C, Gx, dt_stage, max_iters, Piter,
-                                                               resnorm, status, iters, cnt);
+  const StageArgs a{Pn, PE, C, Gx, dt_stage, max_iters, Piter, resnorm, status, iters};
+  newton_stage_kernel<N, G><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
   return 1;
 }
 
@@ -102,47 +127,72 @@ int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, 
 // Otherwise thread t handles zone list[t], t < nlist.  Zones left without a terminal status are appended to
 // next_list (order is not deterministic; the per-zone results are).
 // ---------------------------------------------------------------------------------------------------------
+struct InvertArgs {
+  long long nz, nlist;
+  const long long *list;
+  const double *Ustar;
+  double *Pio;
+  int32_t *iters, *status;
+  double *resnorm;
+  int max_iters, first;
+  long long *next_list;
+};
+
+// One zone of the standalone inversion under arithmetic policy A; same protocol as stage_zone.
+template <int N, class A>
+__device__ __forceinline__ int invert_zone(A &ar, const GridView &gv, const InvertArgs &a, long long z, double *sj) {
+  InvertProblem<N> prob;
+  prob.m = gv.m;
+  prob.tau_ = gv.tau_const;
+  double P[N];
+#pragma unroll
+  for (int v = 0; v < N; v++) {
+    prob.Ustar[v] = a.Ustar[v * a.nz + z];
+    P[v] = a.Pio[v * a.nz + z];
+  }
+  prob.setup(ar);
+  int it = a.first ? 0 : a.iters[z];
+  int st = a.first ? 0 : a.status[z];
+  int nbt = 0;
+  JacView<N, NB> jac{sj};
+  double rn = newton_zone<N, NB>(ar, prob, gv.sp, gv.sp.rtol, P, it, st, a.max_iters, jac, nbt);
+  if (!ar.good()) return -1;
+#pragma unroll
+  for (int v = 0; v < N; v++) a.Pio[v * a.nz + z] = P[v];
+  a.resnorm[z] = rn;
+  a.status[z] = st;
+  a.iters[z] = it;
+  return (nbt << 1) | ((st & ST_TERMINAL) ? 0 : 1);
+}
+
+template <int N>
+__device__ __noinline__ int invert_zone_replay(const GridView &gv, const InvertArgs &a, long long z, double *sj) {
+  ExactArith ar;
+  return invert_zone<N>(ar, gv, a, z, sj);
+}
+
 template <int N>
 __global__ void __launch_bounds__(NB, 2)
-invert_kernel(GridView gv, long long nz, long long nlist, const long long *__restrict__ list,
-              const double *__restrict__ Ustar, double *__restrict__ Pio, int32_t *__restrict__ iters,
-              int32_t *__restrict__ status, double *__restrict__ resnorm, int max_iters, int first,
-              long long *__restrict__ next_list, Counters *cnt) {
+invert_kernel(const __grid_constant__ GridView gv, const __grid_constant__ InvertArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
-  int nbt = 0, active_after = 0;
+  int res = 0;
   long long z = -1;
-  if (t < nlist) {
-    z = first ? t : list[t];
-    InvertProblem<N> prob;
-    prob.m = gv.m;
-    prob.tau_ = gv.tau_const;
-    double P[N];
-#pragma unroll
-    for (int v = 0; v < N; v++) {
-      prob.Ustar[v] = Ustar[v * nz + z];
-      P[v] = Pio[v * nz + z];
-    }
-    prob.setup();
-    int it = first ? 0 : iters[z];
-    int st = first ? 0 : status[z];
-    JacView<N, NB> jac{smem + threadIdx.x};
-    double rn = newton_zone<N, NB>(prob, gv.sp, gv.sp.rtol, P, it, st, max_iters, jac, nbt);
-#pragma unroll
-    for (int v = 0; v < N; v++) Pio[v * nz + z] = P[v];
-    resnorm[z] = rn;
-    status[z] = st;
-    iters[z] = it;
-    active_after = (st & ST_TERMINAL) ? 0 : 1;
+  if (t < a.nlist) {
+    z = a.first ? t : a.list[t];
+    SpecArith ar;
+    res = invert_zone<N>(ar, gv, a, z, smem + threadIdx.x);
+    if (res < 0) res = invert_zone_replay<N>(gv, a, z, smem + threadIdx.x);
   }
+  const int active_after = res & 1;
   // warp-aggregated append to the next active list
   const unsigned ballot = __ballot_sync(0xffffffffu, active_after);
   const int lane = threadIdx.x & 31;
   unsigned long long base = 0;
   if (lane == 0 && ballot) base = atomicAdd(&cnt->list_count, (unsigned long long)__popc(ballot));
   base = __shfl_sync(0xffffffffu, base, 0);
-  if (active_after) next_list[base + __popc(ballot & ((1u << lane) - 1u))] = z;
-  unsigned long long b = __reduce_add_sync(0xffffffffu, (unsigned)nbt);
+  if (active_after) a.next_list[base + __popc(ballot & ((1u << lane) - 1u))] = z;
+  unsigned long long b = __reduce_add_sync(0xffffffffu, (unsigned)(res >> 1));
   if (lane == 0 && b) atomicAdd(&cnt->backtracks, b);
 }
 
@@ -158,8 +208,8 @@ static int launch_invert_t(const GridView &gv, long long nz, long long nlist, co
   }
   const long long blocks = (nlist + NB - 1) / NB;
   if (blocks == 0) return 0;
-  invert_kernel<N><<<(unsigned)blocks, NB, smem, s>>>(gv, nz, nlist, list, Ustar, P, iters, status, resnorm,
-                                                      max_iters, first, next_list, cnt);
+  const InvertArgs a{nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list};
+  invert_kernel<N><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
   return 1;
 }
 
@@ -182,7 +232,8 @@ __global__ void prim_to_conserved_kernel(GridView gv, long long nz, const double
   for (int v = 0; v < N; v++) P[v] = Pin[v * nz + z];
   Pieces pc;
   GeomFlat g;
-  full_state<N>(gv.m, g, gv.tau_const, P, pc.th, pc.v, pc.b, pc.h);
+  ExactArith ar;
+  full_state<N>(ar, gv.m, g, gv.tau_const, P, pc.th, pc.v, pc.b, pc.h);
   flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
 #pragma unroll
   for (int v = 0; v < N; v++) Uout[v * nz + z] = U[v];

@@ -42,16 +42,16 @@ __device__ __forceinline__ double norm2sq(const double (&R)[N]) {
 }
 
 // Residual at P with every piece recomputed; the pieces are returned for reuse.
-template <int N, class Prob>
-__device__ __forceinline__ void eval_full(const Prob &prob, const double (&P)[N], Pieces &pc, double (&R)[N]) {
-  full_state<N>(prob.model(), prob.geom(), prob.tau(), P, pc.th, pc.v, pc.b, pc.h);
+template <int N, class A, class Prob>
+__device__ __forceinline__ void eval_full(A &ar, const Prob &prob, const double (&P)[N], Pieces &pc, double (&R)[N]) {
+  full_state<N>(ar, prob.model(), prob.geom(), prob.tau(), P, pc.th, pc.v, pc.b, pc.h);
   prob.assemble(P, pc, R);
 }
 
 // Residual at P with component J replaced by pj (eq 23): only the pieces that depend on component J are
 // recomputed; the others are those of the unperturbed state.
-template <int J, int N, class Prob>
-__device__ __forceinline__ void eval_column(const Prob &prob, const double (&P)[N], double pj, const Pieces &base,
+template <int J, int N, class A, class Prob>
+__device__ __forceinline__ void eval_column(A &ar, const Prob &prob, const double (&P)[N], double pj, const Pieces &base,
                                             double (&R)[N]) {
   double Pe[N];
 #pragma unroll
@@ -59,14 +59,14 @@ __device__ __forceinline__ void eval_column(const Prob &prob, const double (&P)[
   Pe[J] = pj;
   Pieces pc = base;
   if constexpr (J == RHO || J == UU) {
-    thermo_state<N>(prob.model(), prob.tau(), Pe[RHO], Pe[UU], pc.th);
+    thermo_state<N>(ar, prob.model(), prob.tau(), Pe[RHO], Pe[UU], pc.th);
   } else if constexpr (J >= U1 && J <= U3) {
-    vel_state(prob.geom(), Pe[U1], Pe[U2], Pe[U3], pc.v);
-    mag_state(prob.geom(), pc.v, Pe[B1], Pe[B2], Pe[B3], pc.b);
-    if constexpr (N == 10) bhat_state(pc.b, pc.h);
+    vel_state(ar, prob.geom(), Pe[U1], Pe[U2], Pe[U3], pc.v);
+    mag_state(ar, prob.geom(), pc.v, Pe[B1], Pe[B2], Pe[B3], pc.b);
+    if constexpr (N == 10) bhat_state(ar, pc.b, pc.h);
   } else if constexpr (J >= B1 && J <= B3) {
-    mag_state(prob.geom(), pc.v, Pe[B1], Pe[B2], Pe[B3], pc.b);
-    if constexpr (N == 10) bhat_state(pc.b, pc.h);
+    mag_state(ar, prob.geom(), pc.v, Pe[B1], Pe[B2], Pe[B3], pc.b);
+    if constexpr (N == 10) bhat_state(ar, pc.b, pc.h);
   }
   prob.assemble(Pe, pc, R);
 }
@@ -81,39 +81,39 @@ struct JacView {
 };
 
 // One finite-difference column (eqs 22-23): J[:,j] = (R(P_eps,j) - R0) / (P_eps,j - P_j)
-template <int J, int N, int BLOCK, class Prob>
-__device__ __forceinline__ void fd_column(const Prob &prob, const SolverParams &sp, const double (&P)[N],
+template <int J, int N, int BLOCK, class A, class Prob>
+__device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverParams &sp, const double (&P)[N],
                                           const Pieces &base, const double (&R0)[N], const JacView<N, BLOCK> &jac,
                                           bool &singular) {
   double pj = (fabs(P[J]) < 5.0 * sp.fd_eps) ? sp.fd_eps : (1.0 + sp.fd_eps) * P[J];
   double h = pj - P[J];
   if (h == 0.0) singular = true;
-  double ih = drcp(h);
+  double ih = ar.rcp(h);
   double Rt[N];
-  eval_column<J, N>(prob, P, pj, base, Rt);
+  eval_column<J, N>(ar, prob, P, pj, base, Rt);
 #pragma unroll
   for (int i = 0; i < N; i++) jac.at(JacView<N, BLOCK>::row(i), J) = (Rt[i] - R0[i]) * ih;
 }
 
-template <int J, int N, int BLOCK, class Prob>
+template <int J, int N, int BLOCK, class A, class Prob>
 struct FdColumns {
-  static __device__ __forceinline__ void run(const Prob &prob, const SolverParams &sp, const double (&P)[N],
+  static __device__ __forceinline__ void run(A &ar, const Prob &prob, const SolverParams &sp, const double (&P)[N],
                                              const Pieces &base, const double (&R0)[N],
                                              const JacView<N, BLOCK> &jac, bool &singular) {
-    fd_column<J, N, BLOCK>(prob, sp, P, base, R0, jac, singular);
-    FdColumns<J + 1, N, BLOCK, Prob>::run(prob, sp, P, base, R0, jac, singular);
+    fd_column<J, N, BLOCK>(ar, prob, sp, P, base, R0, jac, singular);
+    FdColumns<J + 1, N, BLOCK, A, Prob>::run(ar, prob, sp, P, base, R0, jac, singular);
   }
 };
-template <int N, int BLOCK, class Prob>
-struct FdColumns<N, N, BLOCK, Prob> {
-  static __device__ __forceinline__ void run(const Prob &, const SolverParams &, const double (&)[N], const Pieces &,
+template <int N, int BLOCK, class A, class Prob>
+struct FdColumns<N, N, BLOCK, A, Prob> {
+  static __device__ __forceinline__ void run(A &, const Prob &, const SolverParams &, const double (&)[N], const Pieces &,
                                              const double (&)[N], const JacView<N, BLOCK> &, bool &) {}
 };
 
 // Solves J x = b (b in, x out) for the Jacobian held in shared memory.  Returns false if a pivot is zero or
 // non-finite (C-19).
-template <int N, int BLOCK>
-__device__ __forceinline__ bool lu_solve(const JacView<N, BLOCK> &jac, double (&b)[N]) {
+template <int N, int BLOCK, class A>
+__device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, double (&b)[N]) {
   int rowoff[N];
   double rinv[N];
 #pragma unroll
@@ -154,7 +154,7 @@ __device__ __forceinline__ bool lu_solve(const JacView<N, BLOCK> &jac, double (&
         int o = rowoff[j]; rowoff[j] = rowoff[i]; rowoff[i] = o;
       }
     }
-    double r = drcp(x[j]);
+    double r = ar.rcp(x[j]);
     rinv[j] = r;
 #pragma unroll
     for (int i = j + 1; i < N; i++) x[i] = x[i] * r;
@@ -173,32 +173,33 @@ __device__ __forceinline__ bool lu_solve(const JacView<N, BLOCK> &jac, double (&
 }
 
 // eq 25 (L230): minimiser of the quadratic through f(0), f'(0) = -2 f(0), f(lam)
-__device__ __forceinline__ double linesearch_lambda(double f0, double flam, double lam) {
-  return ddiv(f0, flam + (2.0 * lam - 1.0) * f0) * lam * lam;
+template <class A>
+__device__ __forceinline__ double linesearch_lambda(A &ar, double f0, double flam, double lam) {
+  return ar.div(f0, flam + (2.0 * lam - 1.0) * f0) * lam * lam;
 }
 
 // Runs at most max_iters further Newton iterations (<= 0: until terminal) of one zone.  P, iters, status carry
 // the zone's state between calls.  Returns ||R(P)||_2 of the final state.
-template <int N, int BLOCK, class Prob>
-__device__ __forceinline__ double newton_zone(const Prob &prob, const SolverParams &sp, double tol, double (&P)[N],
+template <int N, int BLOCK, class A, class Prob>
+__device__ __forceinline__ double newton_zone(A &ar, const Prob &prob, const SolverParams &sp, double tol, double (&P)[N],
                                               int &iters, int &status, int max_iters,
                                               const JacView<N, BLOCK> &jac, int &backtracks) {
   double R0[N];
   Pieces pc;
   int k = iters, st = status, done = 0;
-  eval_full<N>(prob, P, pc, R0);
+  eval_full<N>(ar, prob, P, pc, R0);
   double f0 = norm2sq<N>(R0);
   if (!isfinite(f0)) {
     status = st | ST_NONFINITE;
-    return dsqrt(f0);
+    return ExactArith().sqrt(f0);
   }
-  while (!(dsqrt(f0) < tol) && k < sp.kmax && (max_iters <= 0 || done < max_iters)) {
+  while (!(ar.sqrt_z(f0) < tol) && k < sp.kmax && (max_iters <= 0 || done < max_iters)) {
     bool singular = false;
-    FdColumns<0, N, BLOCK, Prob>::run(prob, sp, P, pc, R0, jac, singular);
+    FdColumns<0, N, BLOCK, A, Prob>::run(ar, prob, sp, P, pc, R0, jac, singular);
     double dP[N];
 #pragma unroll
     for (int v = 0; v < N; v++) dP[v] = -R0[v];
-    bool ok = lu_solve<N, BLOCK>(jac, dP);
+    bool ok = lu_solve<N, BLOCK>(ar, jac, dP);
     if (singular || !ok) {
       st |= ST_SINGULAR;
       break;
@@ -209,15 +210,15 @@ __device__ __forceinline__ double newton_zone(const Prob &prob, const SolverPara
     for (int ls = 0; ls <= sp.lsmax; ls++) {
 #pragma unroll
       for (int v = 0; v < N; v++) Pt[v] = P[v] + lam * dP[v];
-      eval_full<N>(prob, Pt, pc, Rt);
+      eval_full<N>(ar, prob, Pt, pc, Rt);
       ft = norm2sq<N>(Rt);
-      if (dsqrt(ft) < dsqrt(f0) * (1.0 - sp.eps_bt * lam)) {
+      if (isfinite(ft) && ar.sqrt_z(ft) < ar.sqrt_z(f0) * (1.0 - sp.eps_bt * lam)) {
         accepted = true;
         break;
       }
       if (ls == sp.lsmax) break;
       backtracks++;
-      lam = isfinite(ft) ? linesearch_lambda(f0, ft, lam) : 0.5 * lam;
+      lam = isfinite(ft) ? linesearch_lambda(ar, f0, ft, lam) : 0.5 * lam;
     }
     if (!accepted) st |= ST_LS_EXHAUSTED;
 #pragma unroll
@@ -234,12 +235,12 @@ __device__ __forceinline__ double newton_zone(const Prob &prob, const SolverPara
     }
   }
   if (!(st & (ST_SINGULAR | ST_NONFINITE))) {
-    if (dsqrt(f0) < tol) st |= ST_CONVERGED;
+    if (ar.sqrt_z(f0) < tol) st |= ST_CONVERGED;
     else if (k >= sp.kmax) st |= ST_KMAX;
   }
   iters = k;
   status = st;
-  return dsqrt(f0);
+  return ar.sqrt_z(f0);
 }
 
 }  // namespace grim

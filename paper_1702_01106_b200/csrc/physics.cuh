@@ -87,13 +87,13 @@ __device__ __forceinline__ void lower(const G &g, const double (&vcon)[4], doubl
 }
 
 // W = sqrt(1 + g_ij u~^i u~^j); u^t = W/alpha; u^i = u~^i - W beta^i/alpha (C-9)
-template <class G>
-__device__ __forceinline__ void vel_state(const G &g, double ut1, double ut2, double ut3, Vel &v) {
+template <class A, class G>
+__device__ __forceinline__ void vel_state(A &ar, const G &g, double ut1, double ut2, double ut3, Vel &v) {
   if constexpr (G::flat) {
     double usq = ut1 * ut1;
     usq = usq + ut2 * ut2;
     usq = usq + ut3 * ut3;
-    double W = dsqrt(1.0 + usq);
+    double W = ar.sqrt(1.0 + usq);
     v.ucon[0] = W;
     v.ucon[1] = ut1;
     v.ucon[2] = ut2;
@@ -105,8 +105,8 @@ __device__ __forceinline__ void vel_state(const G &g, double ut1, double ut2, do
     for (int i = 1; i < 4; i++)
 #pragma unroll
       for (int j = 1; j < 4; j++) usq = usq + g.cov(i, j) * ut[i - 1] * ut[j - 1];
-    double W = dsqrt(1.0 + usq);
-    v.ucon[0] = ddiv(W, g.alpha);
+    double W = ar.sqrt(1.0 + usq);
+    v.ucon[0] = ar.div(W, g.alpha);
 #pragma unroll
     for (int i = 1; i < 4; i++) v.ucon[i] = ut[i - 1] - W * g.bfac[i - 1];
   }
@@ -114,13 +114,13 @@ __device__ __forceinline__ void vel_state(const G &g, double ut1, double ut2, do
 }
 
 // b^t = B^i u_i ; b^i = (B^i + b^t u^i)/u^t (L248)
-template <class G>
-__device__ __forceinline__ void mag_state(const G &g, const Vel &v, double Bx, double By, double Bz, Mag &b) {
+template <class A, class G>
+__device__ __forceinline__ void mag_state(A &ar, const G &g, const Vel &v, double Bx, double By, double Bz, Mag &b) {
   double bt = Bx * v.ucov[1];
   bt = bt + By * v.ucov[2];
   bt = bt + Bz * v.ucov[3];
   b.bcon[0] = bt;
-  double iut = drcp(v.ucon[0]);
+  double iut = ar.rcp(v.ucon[0]);
   b.bcon[1] = (Bx + bt * v.ucon[1]) * iut;
   b.bcon[2] = (By + bt * v.ucon[2]) * iut;
   b.bcon[3] = (Bz + bt * v.ucon[3]) * iut;
@@ -132,8 +132,9 @@ __device__ __forceinline__ void mag_state(const G &g, const Vel &v, double Bx, d
   b.bsq = bsq;
 }
 
-__device__ __forceinline__ void bhat_state(const Mag &b, BHat &h) {
-  double ibn = drcp(dsqrt(b.bsq));
+template <class A>
+__device__ __forceinline__ void bhat_state(A &ar, const Mag &b, BHat &h) {
+  double ibn = ar.rcp(ar.sqrt(b.bsq));
 #pragma unroll
   for (int i = 0; i < 4; i++) {
     h.con[i] = b.bcon[i] * ibn;
@@ -142,23 +143,24 @@ __device__ __forceinline__ void bhat_state(const Mag &b, BHat &h) {
 }
 
 // c_s^2 = gam P_g/(rho + gam u) (eq 45; L501)
-__device__ __forceinline__ double sound_speed2(const ModelParams &m, double rho, double u) {
+template <class A>
+__device__ __forceinline__ double sound_speed2(A &ar, const ModelParams &m, double rho, double u) {
   double Pg = m.gm1 * u;
-  return ddiv(m.gam * Pg, rho + m.gam * u);
+  return ar.div(m.gam * Pg, rho + m.gam * u);
 }
 
 // eqs 41-42 (L291-293): q~ = q sqrt(tau/(chi rho Theta^2)), dP~ = dP sqrt(tau/(nu rho Theta)), closure of the
 // same state (C-4): chi = phi cs^2 tau, nu = psi cs^2 tau (L299)
-template <int N>
-__device__ __forceinline__ void thermo_state(const ModelParams &m, double tau, double rho, double u, Thermo &t) {
+template <int N, class A>
+__device__ __forceinline__ void thermo_state(A &ar, const ModelParams &m, double tau, double rho, double u, Thermo &t) {
   t.Pg = m.gm1 * u;
   if constexpr (N == 10) {
-    t.Th = ddiv(t.Pg, rho);
-    double cs2 = ddiv(m.gam * t.Pg, rho + m.gam * u);
+    t.Th = ar.div(t.Pg, rho);
+    double cs2 = ar.div(m.gam * t.Pg, rho + m.gam * u);
     double chi = m.phi * cs2 * tau;
     double nu = m.psi * cs2 * tau;
-    t.fq = dsqrt(ddiv(tau, chi * rho * t.Th * t.Th));
-    t.fdp = dsqrt(ddiv(tau, nu * rho * t.Th));
+    t.fq = ar.sqrt(ar.div(tau, chi * rho * t.Th * t.Th));
+    t.fdp = ar.sqrt(ar.div(tau, nu * rho * t.Th));
   } else {
     t.Th = 0.0;
     t.fq = 0.0;
@@ -226,34 +228,34 @@ __device__ __forceinline__ void flux_vector(const G &g, int mu, const double (&P
 }
 
 // Full state of P in one call
-template <int N, class G>
-__device__ __forceinline__ void full_state(const ModelParams &m, const G &g, double tau, const double (&P)[N],
+template <int N, class A, class G>
+__device__ __forceinline__ void full_state(A &ar, const ModelParams &m, const G &g, double tau, const double (&P)[N],
                                            Thermo &th, Vel &v, Mag &b, BHat &h) {
-  vel_state(g, P[U1], P[U2], P[U3], v);
-  mag_state(g, v, P[B1], P[B2], P[B3], b);
-  if constexpr (N == 10) bhat_state(b, h);
-  thermo_state<N>(m, tau, P[RHO], P[UU], th);
+  vel_state(ar, g, P[U1], P[U2], P[U3], v);
+  mag_state(ar, g, v, P[B1], P[B2], P[B3], b);
+  if constexpr (N == 10) bhat_state(ar, b, h);
+  thermo_state<N>(ar, m, tau, P[RHO], P[UU], th);
 }
 
 // v_max^2 (eqs 43-48; eq 46 rather than the simplified eq 49)
-template <int N>
-__device__ __forceinline__ double vmax2(const ModelParams &m, double tau, double rho, double u, double bsq) {
-  double cs2 = sound_speed2(m, rho, u);
-  double va2 = ddiv(bsq, rho + m.gam * u + bsq);
+template <int N, class A>
+__device__ __forceinline__ double vmax2(A &ar, const ModelParams &m, double tau, double rho, double u, double bsq) {
+  double cs2 = sound_speed2(ar, m, rho, u);
+  double va2 = ar.div_z(bsq, rho + m.gam * u + bsq);
   double cst2 = cs2;
   if constexpr (N == 10) {
     double chi = m.phi * cs2 * tau, nu = m.psi * cs2 * tau;
-    double vq2 = ddiv(m.gm1 * chi, tau);
-    double vdp2 = ddiv(4.0 * nu, 3.0 * tau);
-    cst2 = 0.5 * (cs2 + vq2 + dsqrt(cs2 * cs2 + vq2 * vq2)) + vdp2;
+    double vq2 = ar.div(m.gm1 * chi, tau);
+    double vdp2 = ar.div(4.0 * nu, 3.0 * tau);
+    cst2 = 0.5 * (cs2 + vq2 + ar.sqrt(cs2 * cs2 + vq2 * vq2)) + vdp2;
   }
   return cst2 + va2 - cst2 * va2;
 }
 
 // Grid-frame bound along direction d (1..3) of waves moving at +-v_max in the fluid frame (L303; O-4):
 // (k.u)^2 = vmax^2 (g^{mn} + u^m u^n) k_m k_n, k = (-v, delta^d)
-template <class G>
-__device__ __forceinline__ double cmax_dir(const G &g, double vm2, double ut, double ud) {
+template <class A, class G>
+__device__ __forceinline__ double cmax_dir(A &ar, const G &g, double vm2, double ut, double ud) {
   double g00, g0d, gdd;
   if constexpr (G::flat) {
     g00 = -1.0;
@@ -264,13 +266,13 @@ __device__ __forceinline__ double cmax_dir(const G &g, double vm2, double ut, do
     g0d = g.gcon0d;
     gdd = g.gcondd;
   }
-  double A = ut * ut - (g00 + ut * ut) * vm2;
-  double B = 2.0 * (ud * ut - (g0d + ud * ut) * vm2);
-  double C = ud * ud - (gdd + ud * ud) * vm2;
-  double disc = dsqrt(fmax(B * B - 4.0 * A * C, 0.0));
-  double i2A = drcp(2.0 * A);
-  double vp = (B + disc) * i2A;
-  double vn = (B - disc) * i2A;
+  double qa = ut * ut - (g00 + ut * ut) * vm2;
+  double qb = 2.0 * (ud * ut - (g0d + ud * ut) * vm2);
+  double qc = ud * ud - (gdd + ud * ud) * vm2;
+  double disc = ar.sqrt_z(fmax(qb * qb - 4.0 * qa * qc, 0.0));
+  double i2A = ar.rcp(2.0 * qa);
+  double vp = (qb + disc) * i2A;
+  double vn = (qb - disc) * i2A;
   return fmax(fabs(vp), fabs(vn));
 }
 

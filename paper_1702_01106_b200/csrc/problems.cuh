@@ -26,14 +26,15 @@ struct StageProblem {
   __device__ __forceinline__ double tau() const { return tau_; }
 
   // Everything that depends only on P_n and P_E (L438)
-  __device__ __forceinline__ void setup(const double (&Pn)[N], const double (&PE)[N], double dt_stage) {
-    idt = drcp(dt_stage);
-    itau = drcp(tau_);
+  template <class A>
+  __device__ __forceinline__ void setup(A &ar, const double (&Pn)[N], const double (&PE)[N], double dt_stage) {
+    idt = ar.rcp(dt_stage);
+    itau = ar.rcp(tau_);
     Pieces pn;
-    full_state<N>(m, g, tau_, Pn, pn.th, pn.v, pn.b, pn.h);
+    full_state<N>(ar, m, g, tau_, Pn, pn.th, pn.v, pn.b, pn.h);
     double Un[N];
     flux_vector<N>(g, 0, Pn, pn.th, pn.v, pn.b, pn.h, Un);
-    scale = dsqrt(norm2sq<N>(Un)) * idt;
+    scale = ar.sqrt_z(norm2sq<N>(Un)) * idt;
     if constexpr (N == 10) {
       Thn = pn.th.Th;
 #pragma unroll
@@ -42,12 +43,12 @@ struct StageProblem {
       qtn = Pn[QQ] * pn.th.fq;
       dtn = Pn[DPP] * pn.th.fdp;
       Pieces pe;
-      full_state<N>(m, g, tau_, PE, pe.th, pe.v, pe.b, pe.h);
+      full_state<N>(ar, m, g, tau_, PE, pe.th, pe.v, pe.b, pe.h);
 #pragma unroll
       for (int i = 0; i < 4; i++) bh[i] = pe.h.con[i];
       ThE = pe.th.Th;
       utE = pe.v.ucon[0];
-      double cs2 = sound_speed2(m, PE[RHO], PE[UU]);
+      double cs2 = sound_speed2(ar, m, PE[RHO], PE[UU]);
       double chi = m.phi * cs2 * tau_, nu = m.psi * cs2 * tau_;
       nrhochi = -(PE[RHO] * chi);
       rhonu3 = 3.0 * PE[RHO] * nu;
@@ -105,9 +106,10 @@ struct InvertProblem {
   __device__ __forceinline__ const GeomFlat &geom() const { return g; }
   __device__ __forceinline__ double tau() const { return tau_; }
 
-  __device__ __forceinline__ void setup() {
+  template <class A>
+  __device__ __forceinline__ void setup(A &ar) {
     double s2 = norm2sq<N>(Ustar);
-    iscale = drcp(dsqrt(s2));
+    iscale = ar.rcp(ar.sqrt(s2));
   }
   __device__ __forceinline__ void assemble(const double (&P)[N], const Pieces &pc, double (&R)[N]) const {
     double U[N];

@@ -32,9 +32,10 @@ __device__ __forceinline__ double limited_slope(double theta, double vm, double 
 }
 
 // MP5 value at the i+1/2 face from v_{i-2..i+2}; alpha = 4, eps = 1e-10 (C-6)
-__device__ __forceinline__ double mp5_face(double vm2, double vm1, double v0, double vp1, double vp2) {
+template <class A>
+__device__ __forceinline__ double mp5_face(A &ar, double vm2, double vm1, double v0, double vp1, double vp2) {
   const double alpha = 4.0, eps = 1e-10;
-  double vor = ddiv(2.0 * vm2 - 13.0 * vm1 + 47.0 * v0 + 27.0 * vp1 - 3.0 * vp2, 60.0);
+  double vor = div60(ar, 2.0 * vm2 - 13.0 * vm1 + 47.0 * v0 + 27.0 * vp1 - 3.0 * vp2);
   double vmp = v0 + minmod2(vp1 - v0, alpha * (v0 - vm1));
   if ((vor - v0) * (vor - vmp) <= eps) return vor;
   double dm1 = vm2 - 2.0 * vm1 + v0;
@@ -53,12 +54,12 @@ __device__ __forceinline__ double mp5_face(double vm2, double vm1, double v0, do
 
 // v[0..4] = P_{i-2..i+2}.  hi = P^-_{i+1/2} (left state of the upper face), lo = P^+_{i-1/2} (right state of
 // the lower face) (L158-160)
-template <int RECON>
-__device__ __forceinline__ void reconstruct(double theta, double vm2, double vm1, double v0, double vp1, double vp2,
+template <int RECON, class A>
+__device__ __forceinline__ void reconstruct(A &ar, double theta, double vm2, double vm1, double v0, double vp1, double vp2,
                                             double &hi, double &lo) {
   if constexpr (RECON == 1) {
-    hi = mp5_face(vm2, vm1, v0, vp1, vp2);
-    lo = mp5_face(vp2, vp1, v0, vm1, vm2);
+    hi = mp5_face(ar, vm2, vm1, v0, vp1, vp2);
+    lo = mp5_face(ar, vp2, vp1, v0, vm1, vm2);
   } else {
     double s = limited_slope(theta, vm1, v0, vp1);
     hi = v0 + 0.5 * s;
