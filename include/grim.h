@@ -141,6 +141,8 @@ int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_target, cons
 
 /* One time step (a8: L113-148, eq 19 then eq 13; O-11): ghost fill, stage 1 (P_E = P_n, dt' = dt/2, guess P_n),
  * ghost fill, stage 2 (P_E = P_{n+1/2}, dt' = dt, guess P_{n+1/2}); P_inout interior is overwritten by P_{n+1}.
+ * Ghost zones of P_inout on return are those the first ghost fill gave P_n (every call refills them; ghosts of a
+ * GRIM_BC_NONE side are the caller's and are used unchanged for both stages).
  *   dt <= 0: dt = cfl / max_z sum_d c^d/dX^d (C-15).   dt_used : host or NULL.   stats : host or NULL
  * (requesting dt_used or stats synchronises the stream). */
 int grim_timestep(grim_ctx *c, double *P_inout, double dt, double *dt_used, grim_step_stats *stats);

@@ -346,7 +346,7 @@ extern "C" int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_
   if (!(dt_stage > 0.0)) return fail(c, GRIM_EINVAL, "dt_stage must be positive");
   CU(cudaSetDevice(c->d.device));
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
-  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, dt_stage, max_iters, P_iter,
+  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, P_iter, 0, dt_stage, max_iters, P_iter,
                                      resnorm, status, iters, c->cnt, c->stream); });
   rc = check_launch(c, "newton_stage kernel");
   if (rc) return rc;
@@ -436,33 +436,38 @@ extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used,
   }
   if (stats) CU(cudaMemsetAsync(c->stats, 0, 2 * sizeof(StatsDev), s));
 
+  // Ghost zones of a direction whose boundary condition is GRIM_BC_NONE are the caller's: the stage buffer then
+  // starts as a copy of P so that it carries them.  Otherwise each stage reads its guess from P_E and writes the
+  // interior of its output, and nothing is copied.
+  bool caller_ghosts = false;
+  for (int a = 0; a < 3; a++)
+    for (int sd = 0; sd < 2; sd++)
+      if (gv.ngd[a] > 0 && c->d.bc[a][sd] == GRIM_BC_NONE) caller_ghosts = true;
+
   // stage 1: P_E = P_n, dt' = dt/2, guess P_n (eq 19; C-7)
   const double dt1 = 0.5 * dt;
   c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, P, P, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s); });
-  CU(cudaMemcpyAsync(c->Ph, P, pbytes, cudaMemcpyDeviceToDevice, s));
-  CU(cudaMemsetAsync(c->status, 0, (size_t)gv.zg * 4, s));
-  CU(cudaMemsetAsync(c->iters, 0, (size_t)gv.zg * 4, s));
+  if (caller_ghosts) CU(cudaMemcpyAsync(c->Ph, P, pbytes, cudaMemcpyDeviceToDevice, s));
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
-  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, P, c->C, c->G, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s); });
+  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, P, c->C, c->G, P, 1, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s); });
   if (stats) {
     c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_stats(gv, P, dt1, c->resnorm, c->status, c->iters, &c->stats[0], s); });
     CU(cudaMemcpyAsync(&bt[0], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));
   }
-  // stage 2: P_E = P_{n+1/2}, dt' = dt, guess P_{n+1/2} (eq 13)
+  // stage 2: P_E = P_{n+1/2}, dt' = dt, guess P_{n+1/2} (eq 13).  The Newton kernel reads P_n zone by zone
+  // before it writes that zone, so P_{n+1} goes straight into P -- unless the statistics still need P_n.
   c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(gv, c->d.bc, c->Ph, s); });
   c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, c->Ph, P, dt, c->C, c->G, c->Fface, c->cface, nullptr, s); });
-  CU(cudaMemcpyAsync(c->Pnew, c->Ph, pbytes, cudaMemcpyDeviceToDevice, s));
-  CU(cudaMemsetAsync(c->status, 0, (size_t)gv.zg * 4, s));
-  CU(cudaMemsetAsync(c->iters, 0, (size_t)gv.zg * 4, s));
   if (stats) CU(cudaStreamSynchronize(s));  // bt[0] must land before the counters are cleared
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
-  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, c->Ph, c->C, c->G, dt, 0, c->Pnew, c->resnorm, c->status, c->iters,
+  double *out2 = stats ? c->Pnew : P;
+  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, c->Ph, c->C, c->G, c->Ph, 1, dt, 0, out2, c->resnorm, c->status, c->iters,
                                      c->cnt, s); });
   if (stats) {
     c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_stats(gv, P, dt, c->resnorm, c->status, c->iters, &c->stats[1], s); });
     CU(cudaMemcpyAsync(&bt[1], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));
+    c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_copy_interior(gv, c->Pnew, P, s); });
   }
-  CU(cudaMemcpyAsync(P, c->Pnew, pbytes, cudaMemcpyDeviceToDevice, s));
   rc = check_launch(c, "timestep kernels");
   if (rc) return rc;
   if (stats) {

@@ -85,7 +85,7 @@ __device__ __forceinline__ void load_geom(const double *__restrict__ tab, long l
 
 // ---- kernel launchers (defined in the kernels_*.cu files); all enqueue on `s` and return the launch count ----
 int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *G,
-                        double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
+                        const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
                         int32_t *iters, Counters *cnt, cudaStream_t s);
 int launch_invert(const GridView &gv, long long nz, long long nlist, const long long *list, const double *Ustar,
                   double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters, int first,

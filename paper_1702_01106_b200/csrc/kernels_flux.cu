@@ -287,8 +287,11 @@ __device__ __noinline__ void stage_const_replay(const GridView &gv, const double
   for (int v = 0; v < 4; v++) sp_loc[v] = s_[v];
 }
 
+#ifndef GRIM_SC_MINB
+#define GRIM_SC_MINB 4
+#endif
 template <int N, class G>
-__global__ void __launch_bounds__(FB, 4)
+__global__ void __launch_bounds__(FB, GRIM_SC_MINB)
 stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE,
                    const double *__restrict__ Pn, double dt_stage, const double *__restrict__ Fface,
                    const double *__restrict__ cface, double *__restrict__ C, double *__restrict__ Gx,

@@ -11,8 +11,10 @@ static constexpr int NB = 128;  // threads per block; 2 blocks/SM: 2 x 128 x (N*
 
 struct StageArgs {
   const double *Pn, *PE, *C, *Gx;
+  const double *Pguess;  // P^k is read from here and P^k' written to Piter (the two may be the same array)
   double dt_stage;
   int max_iters;
+  int fresh;             // != 0: a new solve; status and iters start at zero without being read
   double *Piter, *resnorm;
   int32_t *status, *iters;
 };
@@ -37,7 +39,7 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
     for (int v = 0; v < N; v++) {
       Pn_z[v] = a.Pn[v * gv.zg + z];
       PE_z[v] = a.PE[v * gv.zg + z];
-      P[v] = a.Piter[v * gv.zg + z];
+      P[v] = a.Pguess[v * gv.zg + z];
       prob.C[v] = a.C[v * gv.zg + z];
     }
     if constexpr (N == 10) {
@@ -48,7 +50,7 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
     prob.setup(ar, Pn_z, PE_z, a.dt_stage);
   }
   const double tol = gv.sp.atol + gv.sp.rtol * prob.scale;
-  int it = a.iters[z];
+  int it = a.fresh ? 0 : a.iters[z];
   int nbt = 0;
   JacView<N, NB> jac{sj};
   double rn = newton_zone<N, NB>(ar, prob, gv.sp, tol, P, it, st, a.max_iters, jac, nbt);
@@ -78,7 +80,7 @@ newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__
     int i, j, k;
     zone_coords(gv, t, i, j, k);
     const long long z = zone_index(gv, i, j, k);
-    const int st = a.status[z];
+    const int st = a.fresh ? 0 : a.status[z];
     if (!(st & ST_TERMINAL)) {
       SpecArith ar;
       res = stage_zone<N, G>(ar, gv, a, z, i, j, st, smem + threadIdx.x);
@@ -96,7 +98,7 @@ newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__
 
 template <int N, class G>
 static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *Gx,
-                          double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
+                          const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
                           int32_t *iters, Counters *cnt, cudaStream_t s) {
   const size_t smem = (size_t)N * N * NB * sizeof(double);
   static bool attr_set = false;
@@ -105,21 +107,21 @@ static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE
     attr_set = true;
   }
   const long long blocks = (gv.nint + NB - 1) / NB;
-  const StageArgs a{Pn, PE, C, Gx, dt_stage, max_iters, Piter, resnorm, status, iters};
+  const StageArgs a{Pn, PE, C, Gx, Pguess, dt_stage, max_iters, fresh, Piter, resnorm, status, iters};
   newton_stage_kernel<N, G><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
   return 1;
 }
 
 int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *G,
-                        double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
+                        const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
                         int32_t *iters, Counters *cnt, cudaStream_t s) {
   const bool flat = (gv.metric == 0);
   if (gv.nvar == 10) {
-    return flat ? launch_stage_t<10, GeomFlat>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
-                : launch_stage_t<10, GeomGen>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
+    return flat ? launch_stage_t<10, GeomFlat>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
+                : launch_stage_t<10, GeomGen>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
   }
-  return flat ? launch_stage_t<8, GeomFlat>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
-              : launch_stage_t<8, GeomGen>(gv, Pn, PE, C, G, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
+  return flat ? launch_stage_t<8, GeomFlat>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
+              : launch_stage_t<8, GeomGen>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
 }
 
 // ---------------------------------------------------------------------------------------------------------
