@@ -25,8 +25,9 @@ struct StageArgs {
 template <int N, class G, class A>
 __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const StageArgs &a, long long z, int i, int j,
                                           int st, double *sj) {
-  StageProblem<N, G> prob;
+  StageProblem<N, G, NB> prob;
   prob.m = gv.m;
+  prob.Cs = sj + N * N * NB;
   if constexpr (G::flat) {
     prob.tau_ = gv.tau_const;
   } else {
@@ -40,7 +41,7 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
       Pn_z[v] = a.Pn[v * gv.zg + z];
       PE_z[v] = a.PE[v * gv.zg + z];
       P[v] = a.Pguess[v * gv.zg + z];
-      prob.C[v] = a.C[v * gv.zg + z];
+      sj[(N * N + v) * NB] = a.C[v * gv.zg + z];
     }
     if constexpr (N == 10) {
       prob.Xq = a.Gx[0 * gv.zg + z];
@@ -100,7 +101,7 @@ template <int N, class G>
 static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *Gx,
                           const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
                           int32_t *iters, Counters *cnt, cudaStream_t s) {
-  const size_t smem = (size_t)N * N * NB * sizeof(double);
+  const size_t smem = (size_t)(N * N + N) * NB * sizeof(double);  // Jacobian + C (or U*) per thread
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(newton_stage_kernel<N, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -143,13 +144,14 @@ struct InvertArgs {
 // One zone of the standalone inversion under arithmetic policy A; same protocol as stage_zone.
 template <int N, class A>
 __device__ __forceinline__ int invert_zone(A &ar, const GridView &gv, const InvertArgs &a, long long z, double *sj) {
-  InvertProblem<N> prob;
+  InvertProblem<N, NB> prob;
   prob.m = gv.m;
+  prob.Us = sj + N * N * NB;
   prob.tau_ = gv.tau_const;
   double P[N];
 #pragma unroll
   for (int v = 0; v < N; v++) {
-    prob.Ustar[v] = a.Ustar[v * a.nz + z];
+    sj[(N * N + v) * NB] = a.Ustar[v * a.nz + z];
     P[v] = a.Pio[v * a.nz + z];
   }
   prob.setup(ar);
@@ -202,7 +204,7 @@ template <int N>
 static int launch_invert_t(const GridView &gv, long long nz, long long nlist, const long long *list,
                            const double *Ustar, double *P, int32_t *iters, int32_t *status, double *resnorm,
                            int max_iters, int first, long long *next_list, Counters *cnt, cudaStream_t s) {
-  const size_t smem = (size_t)N * N * NB * sizeof(double);
+  const size_t smem = (size_t)(N * N + N) * NB * sizeof(double);  // Jacobian + C (or U*) per thread
   static bool attr_set = false;
   if (!attr_set) {
     cudaFuncSetAttribute(invert_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);

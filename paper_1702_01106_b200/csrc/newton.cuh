@@ -111,11 +111,14 @@ struct FdColumns<N, N, BLOCK, A, Prob> {
 };
 
 // Solves J x = b (b in, x out) for the Jacobian held in shared memory.  Returns false if a pivot is zero or
-// non-finite (C-19).
+// non-finite (C-19).  Registers hold one column at a time, in pivoted order: position i of the order is the
+// matrix row at shared-memory offset rowoff[i].  A row exchange exchanges two entries of rowoff and nothing
+// else -- the column in registers dies when it is stored, the right-hand side is permuted once, through the
+// storage of the last column, when the order is final -- and the diagonal slot receives the reciprocal of the
+// pivot, which is all the back substitution needs of it.
 template <int N, int BLOCK, class A>
 __device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, double (&b)[N]) {
   int rowoff[N];
-  double rinv[N];
 #pragma unroll
   for (int i = 0; i < N; i++) rowoff[i] = JacView<N, BLOCK>::row(i);
   bool ok = true;
@@ -124,6 +127,14 @@ __device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, do
     double x[N];
 #pragma unroll
     for (int i = 0; i < N; i++) x[i] = jac.at(rowoff[i], j);
+    if (j == N - 1) {
+      // positions 0..N-2 are final and position N-1 is the row that is left: permute b through this column's
+      // storage, which the loads above have just emptied
+#pragma unroll
+      for (int i = 0; i < N; i++) jac.at(JacView<N, BLOCK>::row(i), j) = b[i];
+#pragma unroll
+      for (int i = 0; i < N; i++) b[i] = jac.at(rowoff[i], j);
+    }
     // updates of the earlier pivots, k ascending; the last column carries the right-hand side along
 #pragma unroll
     for (int k = 0; k < j; k++) {
@@ -134,32 +145,33 @@ __device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, do
         if (j == N - 1) b[i] = b[i] - l * b[k];
       }
     }
-    // pivot: first row of maximal |x_i|, i >= j
-    int p = j;
-    double amax = fabs(x[j]);
+    // pivot: first position of maximal |x_i|, i >= j
+    int p = j, rop = rowoff[j];
+    double xp = x[j], amax = fabs(x[j]);
 #pragma unroll
     for (int i = j + 1; i < N; i++) {
       double v = fabs(x[i]);
       if (v > amax) {
         amax = v;
+        xp = x[i];
         p = i;
+        rop = rowoff[i];
       }
     }
     if (!(amax > 0.0) || !isfinite(amax)) ok = false;
+    double r = ar.rcp(xp);
+    // U above the diagonal; multipliers x_i / pivot for every candidate row (the pivot row's own slot is then
+    // overwritten by 1/pivot)
 #pragma unroll
-    for (int i = j + 1; i < N; i++) {
-      if (p == i) {
-        double t = x[j]; x[j] = x[i]; x[i] = t;
-        t = b[j]; b[j] = b[i]; b[i] = t;
-        int o = rowoff[j]; rowoff[j] = rowoff[i]; rowoff[i] = o;
-      }
-    }
-    double r = ar.rcp(x[j]);
-    rinv[j] = r;
+    for (int i = 0; i < j; i++) jac.at(rowoff[i], j) = x[i];
 #pragma unroll
-    for (int i = j + 1; i < N; i++) x[i] = x[i] * r;
+    for (int i = j; i < N; i++) jac.at(rowoff[i], j) = x[i] * r;
+    jac.at(rop, j) = r;
+    // exchange positions j and p
 #pragma unroll
-    for (int i = 0; i < N; i++) jac.at(rowoff[i], j) = x[i];
+    for (int i = j + 1; i < N; i++)
+      if (p == i) rowoff[i] = rowoff[j];
+    rowoff[j] = rop;
   }
   // back substitution with U
 #pragma unroll
@@ -167,7 +179,7 @@ __device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, do
     double s = b[i];
 #pragma unroll
     for (int j = i + 1; j < N; j++) s = s - jac.at(rowoff[i], j) * b[j];
-    b[i] = s * rinv[i];
+    b[i] = s * jac.at(rowoff[i], i);
   }
   return ok;
 }

@@ -8,13 +8,14 @@
 
 namespace grim {
 
-template <int N, class G>
+// CS: stride (in doubles) of the per-thread shared-memory vector that holds the stage constant C
+template <int N, class G, int CS>
 struct StageProblem {
   ModelParams m;
   G g;
   double tau_, idt, itau;
-  double C[N];
-  double scale;  // ||U(P_n)||_2 / dt' (C-2)
+  const double *Cs;  // C[v] at Cs[v * CS] (shared memory: read once per residual evaluation, 2N registers saved)
+  double scale;      // ||U(P_n)||_2 / dt' (C-2)
   // EMHD only.  P_n-derived:
   double Thn, ucovn[4], utn, qtn, dtn;
   // P_E-derived coefficients, frozen during the iteration (O-8), and the spatial-gradient terms of the stage:
@@ -63,7 +64,7 @@ struct StageProblem {
     double U[N];
     flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
 #pragma unroll
-    for (int v = 0; v < N; v++) R[v] = U[v] * idt + C[v];
+    for (int v = 0; v < N; v++) R[v] = U[v] * idt + Cs[v * CS];
     if constexpr (N == 10) {
       // time derivatives of derived quantities between the unknown state and P_n (C-3)
       double dtTheta = (pc.th.Th - Thn) * idt;
@@ -94,12 +95,12 @@ struct StageProblem {
   }
 };
 
-template <int N>
+template <int N, int CS>
 struct InvertProblem {
   ModelParams m;
   GeomFlat g;
   double tau_;
-  double Ustar[N];
+  const double *Us;  // U*[v] at Us[v * CS] (shared memory)
   double iscale;
 
   __device__ __forceinline__ const ModelParams &model() const { return m; }
@@ -108,6 +109,9 @@ struct InvertProblem {
 
   template <class A>
   __device__ __forceinline__ void setup(A &ar) {
+    double Ustar[N];
+#pragma unroll
+    for (int v = 0; v < N; v++) Ustar[v] = Us[v * CS];
     double s2 = norm2sq<N>(Ustar);
     iscale = ar.rcp(ar.sqrt(s2));
   }
@@ -115,7 +119,7 @@ struct InvertProblem {
     double U[N];
     flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
 #pragma unroll
-    for (int v = 0; v < N; v++) R[v] = (U[v] - Ustar[v]) * iscale;
+    for (int v = 0; v < N; v++) R[v] = (U[v] - Us[v * CS]) * iscale;
   }
 };
 
