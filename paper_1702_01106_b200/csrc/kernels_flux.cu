@@ -16,23 +16,33 @@ namespace grim {
 
 static constexpr int FB = 128;
 
-// LLF flux and face speed of the lower DIR-face of padded zone z under arithmetic policy A
-template <int N, int RECON, class G, int DIR, class A>
-__device__ __forceinline__ void face_compute(A &ar, const GridView &gv, const double *__restrict__ PE, long long z,
-                                             int i, int j, double (&F)[N], double &c) {
-  const long long stride = (DIR == 0) ? 1 : (DIR == 1) ? (long long)gv.sz[0] : (long long)gv.sz[0] * gv.sz[1];
+// Stencil sources of a face: m = 0 .. H-1 counts the zones of the stencil upwards along DIR, H = 6 (MP5:
+// zones i-3 .. i+2 of lower face i) or 4 (minmod: i-2 .. i+1).
+struct GlobalStencil {  // straight from the grid array (replay path)
+  const double *p;      // variable 0 at the lowest zone of the stencil
+  long long stride, zg;
+  __device__ __forceinline__ double operator()(int v, int m) const { return p[v * zg + m * stride]; }
+};
+template <int VS, int MS>
+struct TileStencil {    // from the block's shared-memory tile: variable stride VS, stencil stride MS (doubles)
+  const double *p;
+  __device__ __forceinline__ double operator()(int v, int m) const { return p[v * VS + m * MS]; }
+};
+
+// LLF flux and face speed of one lower DIR-face under arithmetic policy A
+template <int N, int RECON, class G, int DIR, class A, class S>
+__device__ __forceinline__ void face_compute(A &ar, const GridView &gv, const S &st, int i, int j, double (&F)[N],
+                                             double &c) {
   double Pm[N], Pp[N];  // P^- (from zone i-1) and P^+ (from zone i) at the face (L158-160)
 #pragma unroll
   for (int v = 0; v < N; v++) {
-    const double *p = PE + v * gv.zg + z;
     double hi, lo, unused;
     if constexpr (RECON == 1) {
-      const double s0 = p[-3 * stride], s1 = p[-2 * stride], s2 = p[-stride], s3 = p[0], s4 = p[stride],
-                   s5 = p[2 * stride];
+      const double s0 = st(v, 0), s1 = st(v, 1), s2 = st(v, 2), s3 = st(v, 3), s4 = st(v, 4), s5 = st(v, 5);
       hi = mp5_face(ar, s0, s1, s2, s3, s4);
       lo = mp5_face(ar, s5, s4, s3, s2, s1);
     } else {
-      const double s1 = p[-2 * stride], s2 = p[-stride], s3 = p[0], s4 = p[stride];
+      const double s1 = st(v, 0), s2 = st(v, 1), s3 = st(v, 2), s4 = st(v, 3);
       reconstruct<0>(ar, gv.theta, 0.0, s1, s2, s3, 0.0, hi, unused);
       reconstruct<0>(ar, gv.theta, 0.0, s2, s3, s4, 0.0, unused, lo);
     }
@@ -66,11 +76,22 @@ __device__ __noinline__ void face_replay(const GridView &gv, const double *__res
                                          double *__restrict__ Fface, double *__restrict__ cface) {
   ExactArith ar;
   double F[N], c;
-  face_compute<N, RECON, G, DIR>(ar, gv, PE, z, i, j, F, c);
+  const long long stride = (DIR == 0) ? 1 : (DIR == 1) ? (long long)gv.sz[0] : (long long)gv.sz[0] * gv.sz[1];
+  const GlobalStencil st{PE + z - (RECON == 1 ? 3 : 2) * stride, stride, gv.zg};
+  face_compute<N, RECON, G, DIR>(ar, gv, st, i, j, F, c);
 #pragma unroll
   for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
   cface[z] = c;
 }
+
+// Block tile of faces: 128 x 1 x 1 for DIR 0, 32 x 4 x 1 for DIR 1, 32 x 1 x 4 for DIR 2 -- X^1 stays the fast
+// index of every load and store, and the tile is 4 faces deep along DIR so that its stencil zones
+// (tile + H-1 along DIR) are staged once in shared memory and read 6H/(4+H-1) times: one batch of independent
+// coalesced loads per block instead of H dependent-latency loads per variable and thread.
+template <int DIR>
+struct FaceTile {
+  static constexpr int T0 = (DIR == 0) ? 128 : 32, T1 = (DIR == 1) ? 4 : 1, T2 = (DIR == 2) ? 4 : 1;
+};
 
 #ifndef GRIM_FLUX_MINB
 #define GRIM_FLUX_MINB 4
@@ -79,18 +100,73 @@ template <int N, int RECON, class G, int DIR>  // DIR = 0..2
 __global__ void __launch_bounds__(FB, GRIM_FLUX_MINB)
 face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE, double *__restrict__ Fface,
                  double *__restrict__ cface) {
-  // faces: index range [ng, ng+n] along DIR, interior along the other directions
-  const int n0 = gv.n[0] + (DIR == 0), n1 = gv.n[1] + (DIR == 1), n2 = gv.n[2] + (DIR == 2);
-  const long long t = (long long)blockIdx.x * FB + threadIdx.x;
-  if (t >= (long long)n0 * n1 * n2) return;
-  const int i = (int)(t % n0) + gv.ngd[0];
-  const long long r = t / n0;
-  const int j = (int)(r % n1) + gv.ngd[1];
-  const int k = (int)(r / n1) + gv.ngd[2];
+  using T = FaceTile<DIR>;
+  constexpr int H = (RECON == 1) ? 6 : 4, LO = H / 2;
+  constexpr int E0 = T::T0 + (DIR == 0 ? H - 1 : 0), E1 = T::T1 + (DIR == 1 ? H - 1 : 0),
+                E2 = T::T2 + (DIR == 2 ? H - 1 : 0), EZ = E0 * E1 * E2;
+  constexpr int MS = (DIR == 0) ? 1 : (DIR == 1) ? E0 : E0 * E1;
+  __shared__ double tile[N * EZ];
+
+  // padded coordinates of the tile's first face, and of the first staged zone (LO zones below it along DIR)
+  const int fi = gv.ngd[0] + (int)blockIdx.x * T::T0, fj = gv.ngd[1] + (int)blockIdx.y * T::T1,
+            fk = gv.ngd[2] + (int)blockIdx.z * T::T2;
+  const int zi = fi - (DIR == 0 ? LO : 0), zj = fj - (DIR == 1 ? LO : 0), zk = fk - (DIR == 2 ? LO : 0);
+  constexpr int ITER = (EZ + FB - 1) / FB;
+#pragma unroll
+  for (int it = 0; it < ITER; it++) {
+    const int e = it * FB + (int)threadIdx.x;
+    const int e0 = e % E0, e1 = (e / E0) % E1, e2 = e / (E0 * E1);
+    const int ci = zi + e0, cj = zj + e1, ck = zk + e2;
+    if (e < EZ && ci < gv.sz[0] && cj < gv.sz[1] && ck < gv.sz[2]) {
+      const long long zz = zone_index(gv, ci, cj, ck);
+      double tmp[N];
+#pragma unroll
+      for (int v = 0; v < N; v++) tmp[v] = PE[v * gv.zg + zz];
+#pragma unroll
+      for (int v = 0; v < N; v++) tile[v * EZ + e] = tmp[v];
+    }
+  }
+  __syncthreads();
+
+  const int t0 = (int)threadIdx.x % T::T0, t1 = ((int)threadIdx.x / T::T0) % T::T1,
+            t2 = (int)threadIdx.x / (T::T0 * T::T1);
+  const int i = fi + t0, j = fj + t1, k = fk + t2;
+  // the tiles cover the n lower faces of the interior zones; the one upper boundary face per line goes to
+  // face_edge_kernel, so that the tile grid divides the interior evenly
+  if (i >= gv.ngd[0] + gv.n[0] || j >= gv.ngd[1] + gv.n[1] || k >= gv.ngd[2] + gv.n[2]) return;
   const long long z = zone_index(gv, i, j, k);
   SpecArith ar;
   double F[N], c;
-  face_compute<N, RECON, G, DIR>(ar, gv, PE, z, i, j, F, c);
+  const TileStencil<EZ, MS> st{tile + (t2 * E1 + t1) * E0 + t0};
+  face_compute<N, RECON, G, DIR>(ar, gv, st, i, j, F, c);
+  if (ar.good()) {
+#pragma unroll
+    for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
+    cface[z] = c;
+  } else {
+    face_replay<N, RECON, G, DIR>(gv, PE, z, i, j, Fface, cface);
+  }
+}
+
+// The upper boundary faces of direction DIR (face index n along DIR): one thread per face, stencil read
+// directly from the grid array.  1/n of the faces.
+template <int N, int RECON, class G, int DIR>
+__global__ void __launch_bounds__(FB, GRIM_FLUX_MINB)
+face_edge_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE, double *__restrict__ Fface,
+                 double *__restrict__ cface) {
+  const int na = (DIR == 0) ? gv.n[1] : gv.n[0], nb = (DIR == 2) ? gv.n[1] : gv.n[2];  // the plane's extents
+  const long long t = (long long)blockIdx.x * FB + threadIdx.x;
+  if (t >= (long long)na * nb) return;
+  const int ta = (int)(t % na), tb = (int)(t / na);
+  const int i = (DIR == 0) ? gv.ngd[0] + gv.n[0] : gv.ngd[0] + ta;
+  const int j = (DIR == 0) ? gv.ngd[1] + ta : (DIR == 1) ? gv.ngd[1] + gv.n[1] : gv.ngd[1] + tb;
+  const int k = (DIR == 2) ? gv.ngd[2] + gv.n[2] : gv.ngd[2] + tb;
+  const long long z = zone_index(gv, i, j, k);
+  const long long stride = (DIR == 0) ? 1 : (DIR == 1) ? (long long)gv.sz[0] : (long long)gv.sz[0] * gv.sz[1];
+  SpecArith ar;
+  double F[N], c;
+  const GlobalStencil st{PE + z - (RECON == 1 ? 3 : 2) * stride, stride, gv.zg};
+  face_compute<N, RECON, G, DIR>(ar, gv, st, i, j, F, c);
   if (ar.good()) {
 #pragma unroll
     for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
@@ -109,8 +185,9 @@ template <int N, class G, class A>
 __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, const double *__restrict__ PE,
                                                     const double *__restrict__ Pn, double dt_stage,
                                                     const double *__restrict__ Fface,
-                                                    const double *__restrict__ cface, long long z, long long id,
-                                                    double (&Cout)[N], double (&Gout)[3], double (&sp_loc)[4]) {
+                                                    const double *__restrict__ cface, bool want_speeds, long long z,
+                                                    long long id, double (&Cout)[N], double (&Gout)[3],
+                                                    double (&sp_loc)[4]) {
   const double idt = ar.rcp(dt_stage);
   G gc;
   double tau = gv.tau_const;
@@ -142,9 +219,11 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
     const long long zu = z + strides[a];
 #pragma unroll
     for (int v = 0; v < N; v++) divF[v] = divF[v] + (Fa[v * gv.zg + zu] - Fa[v * gv.zg + z]) * gv.idx[a];
-    const double cz = fmax(ca[z], ca[zu]) * gv.idx[a];
-    sp_loc[a] = cz;
-    ssum = ssum + cz;
+    if (want_speeds) {  // only the dt probe needs them (C-15)
+      const double cz = fmax(ca[z], ca[zu]) * gv.idx[a];
+      sp_loc[a] = cz;
+      ssum = ssum + cz;
+    }
   }
   sp_loc[3] = ssum;
 
@@ -277,11 +356,11 @@ template <int N, class G>
 __device__ __noinline__ void stage_const_replay(const GridView &gv, const double *__restrict__ PE,
                                                 const double *__restrict__ Pn, double dt_stage,
                                                 const double *__restrict__ Fface, const double *__restrict__ cface,
-                                                long long z, long long id, double *Cout, double *Gout,
-                                                double *sp_loc) {
+                                                bool want_speeds, long long z, long long id, double *Cout,
+                                                double *Gout, double *sp_loc) {
   ExactArith ar;
   double C_[N], G_[3] = {0.0, 0.0, 0.0}, s_[4] = {0.0, 0.0, 0.0, 0.0};
-  stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, z, id, C_, G_, s_);
+  stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, want_speeds, z, id, C_, G_, s_);
   for (int v = 0; v < N; v++) Cout[v] = C_[v];
   for (int v = 0; v < 3; v++) Gout[v] = G_[v];
   for (int v = 0; v < 4; v++) sp_loc[v] = s_[v];
@@ -305,8 +384,9 @@ stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict
     const long long id = (long long)j * gv.sz[0] + i;
     double Cout[N], Gout[3] = {0.0, 0.0, 0.0};
     SpecArith ar;
-    stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, z, id, Cout, Gout, sp_loc);
-    if (!ar.good()) stage_const_replay<N, G>(gv, PE, Pn, dt_stage, Fface, cface, z, id, Cout, Gout, sp_loc);
+    stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
+    if (!ar.good())
+      stage_const_replay<N, G>(gv, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
 #pragma unroll
     for (int v = 0; v < N; v++) C[v * gv.zg + z] = Cout[v];
     if constexpr (N == 10) {
@@ -332,14 +412,21 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
   int launches = 0;
   for (int a = 0; a < 3; a++) {
     if (gv.ngd[a] == 0) continue;
-    const long long nf = (long long)(gv.n[0] + (a == 0)) * (gv.n[1] + (a == 1)) * (gv.n[2] + (a == 2));
-    const unsigned blocks = (unsigned)((nf + FB - 1) / FB);
+    const int f0 = gv.n[0], f1 = gv.n[1], f2 = gv.n[2];  // tiled faces per direction (+ one edge plane along a)
     double *Fa = Fface + (long long)a * N * gv.zg;
     double *ca = cface + (long long)a * gv.zg;
-    if (a == 0) face_flux_kernel<N, RECON, G, 0><<<blocks, FB, 0, s>>>(gv, PE, Fa, ca);
-    if (a == 1) face_flux_kernel<N, RECON, G, 1><<<blocks, FB, 0, s>>>(gv, PE, Fa, ca);
-    if (a == 2) face_flux_kernel<N, RECON, G, 2><<<blocks, FB, 0, s>>>(gv, PE, Fa, ca);
-    launches++;
+    auto tiles = [&](int t0, int t1, int t2) {
+      return dim3((unsigned)((f0 + t0 - 1) / t0), (unsigned)((f1 + t1 - 1) / t1), (unsigned)((f2 + t2 - 1) / t2));
+    };
+    if (a == 0) face_flux_kernel<N, RECON, G, 0><<<tiles(128, 1, 1), FB, 0, s>>>(gv, PE, Fa, ca);
+    if (a == 1) face_flux_kernel<N, RECON, G, 1><<<tiles(32, 4, 1), FB, 0, s>>>(gv, PE, Fa, ca);
+    if (a == 2) face_flux_kernel<N, RECON, G, 2><<<tiles(32, 1, 4), FB, 0, s>>>(gv, PE, Fa, ca);
+    const long long ne = (long long)f0 * f1 * f2 / gv.n[a];
+    const unsigned eb = (unsigned)((ne + FB - 1) / FB);
+    if (a == 0) face_edge_kernel<N, RECON, G, 0><<<eb, FB, 0, s>>>(gv, PE, Fa, ca);
+    if (a == 1) face_edge_kernel<N, RECON, G, 1><<<eb, FB, 0, s>>>(gv, PE, Fa, ca);
+    if (a == 2) face_edge_kernel<N, RECON, G, 2><<<eb, FB, 0, s>>>(gv, PE, Fa, ca);
+    launches += 2;
   }
   const unsigned blocks = (unsigned)((gv.nint + FB - 1) / FB);
   stage_const_kernel<N, G><<<blocks, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx, cnt);
