@@ -7,7 +7,10 @@
 
 namespace grim {
 
-static constexpr int NB = 128;  // threads per block; 2 blocks/SM: 2 x 128 x (N*N*8 B) of Jacobian + 255 registers
+#ifndef GRIM_NB
+#define GRIM_NB 128
+#endif
+static constexpr int NB = GRIM_NB;  // threads per block; 2 blocks/SM: 2 x 128 x (N*N*8 B) of Jacobian + 255 registers
 
 struct StageArgs {
   const double *Pn, *PE, *C, *Gx;
@@ -72,7 +75,7 @@ __device__ __noinline__ int stage_zone_replay(const GridView &gv, const StageArg
 }
 
 template <int N, class G>
-__global__ void __launch_bounds__(NB, 2)
+__global__ void __launch_bounds__(NB, 256 / NB)
 newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
@@ -176,7 +179,7 @@ __device__ __noinline__ int invert_zone_replay(const GridView &gv, const InvertA
 }
 
 template <int N>
-__global__ void __launch_bounds__(NB, 2)
+__global__ void __launch_bounds__(NB, 256 / NB)
 invert_kernel(const __grid_constant__ GridView gv, const __grid_constant__ InvertArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;

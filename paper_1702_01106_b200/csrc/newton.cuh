@@ -95,12 +95,34 @@ __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverP
   for (int i = 0; i < N; i++) jac.at(JacView<N, BLOCK>::row(i), J) = (Rt[i] - R0[i]) * ih;
 }
 
+// Order in which the (independent) columns are evaluated: first those that reuse every piece of the unperturbed
+// state (q, dP), then the thermodynamic ones (reuse velocity, field, bhat), the field ones (velocity, thermo), last
+// the velocity ones (thermo only) -- so the cached pieces die as early as possible and the later, more expensive
+// columns have the registers.  The Jacobian does not depend on the order.
+#ifndef GRIM_FD_ORDER
+#define GRIM_FD_ORDER 1
+#endif
+template <int N>
+__host__ __device__ constexpr int fd_order(int s) {
+#if GRIM_FD_ORDER == 1
+  constexpr int ord10[10] = {QQ, DPP, RHO, UU, B1, B2, B3, U1, U2, U3};
+  constexpr int ord8[8] = {RHO, UU, B1, B2, B3, U1, U2, U3};
+  return N == 10 ? ord10[s] : ord8[s];
+#elif GRIM_FD_ORDER == 2
+  constexpr int ord10[10] = {U1, U2, U3, B1, B2, B3, RHO, UU, QQ, DPP};
+  constexpr int ord8[8] = {U1, U2, U3, B1, B2, B3, RHO, UU};
+  return N == 10 ? ord10[s] : ord8[s];
+#else
+  return s;
+#endif
+}
+
 template <int J, int N, int BLOCK, class A, class Prob>
 struct FdColumns {
   static __device__ __forceinline__ void run(A &ar, const Prob &prob, const SolverParams &sp, const double (&P)[N],
                                              const Pieces &base, const double (&R0)[N],
                                              const JacView<N, BLOCK> &jac, bool &singular) {
-    fd_column<J, N, BLOCK>(ar, prob, sp, P, base, R0, jac, singular);
+    fd_column<fd_order<N>(J), N, BLOCK>(ar, prob, sp, P, base, R0, jac, singular);
     FdColumns<J + 1, N, BLOCK, A, Prob>::run(ar, prob, sp, P, base, R0, jac, singular);
   }
 };
