@@ -26,9 +26,17 @@ sys.path.insert(0, ROOT)
 METRIC = "fp64 zone-updates/sec per Newton step (EMHD 10-var) and % of HBM roofline"
 UNIT = "zone-updates/s"
 
-# per zone and stage, Minkowski EMHD, 2 Newton iterations (measured with ncu, profiles/)
-ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 6114.0    # fp64-pipe thread instructions of the Newton kernel per zone (ncu, profiles/r1_ncu_full_stage_kernels.md)
+# per zone and stage of the Newton kernel, Minkowski EMHD, 2 Newton iterations.
+# Algorithmic fp64 work: DADD + DMUL + DFMA thread instructions that the method's definition requires under the strict
+# arithmetic contract (every + - * separately rounded, / and sqrt as correctly rounded Newton-Raphson sequences), counted
+# with ncu on the round's first kernel (profiles/r1a_ncu_full_stage_kernels_baseline.md) and then FROZEN, so that later
+# kernels cannot raise the fraction by executing more instructions.  (The current kernel executes 6242 fp64-pipe thread
+# instructions per zone and stage, compares included: profiles/r1g_ncu_full_stage_kernels.md.)
+ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 6114.0
 ALG_BYTES_PER_ZONE_STAGE_NEWTON = 8.0 * (10 + 10 + 10 + 10 + 3 + 10 + 1) + 4 * 4   # P^k,P_n,P_E,C,G in; P,|R| out; status,iters in/out
+# dram__bytes_read.sum + dram__bytes_write.sum of the Newton kernel per zone, mean of the stage-1 and stage-2 launches of
+# one ncu --set full capture (profiles/r1g_ncu_full_stage_kernels.md: 4.82 GB and 6.16 GB per 256^3 launch)
+NCU_DRAM_BYTES_PER_ZONE_STAGE_NEWTON = 327.0
 FP64_INSTR_PER_CLK_PER_SM = 64.0                 # B200: 64 fp64 lanes per SM (guide: unit counts), 148 SMs
 N_SM = 148
 
@@ -218,7 +226,8 @@ def run_ours(args):
                 "d2h_bytes_per_step": pbytes},
         "gpu_launches": int(launches),
         "roofline": {"bound": "alu", "kernel": "newton_stage_kernel<10,flat>", "achieved": alu_ach, "peak": alu_peak,
-                     "unit": "T fp64 instr/s", "frac": alu_ach / alu_peak, "traffic": None,
+                     "unit": "T fp64 instr/s", "frac": alu_ach / alu_peak,
+                     "traffic": NCU_DRAM_BYTES_PER_ZONE_STAGE_NEWTON * zones,
                      "peak_source": "148 SM x 64 fp64 lanes x %s sm_max_mhz %.0f" % (which, sm_max),
                      "launch_ms": newton_ms, "launches": int(nk_n)},
         "roofline_hbm": {"bound": "hbm", "kernel": "newton_stage_kernel<10,flat>", "achieved": hbm_ach,
@@ -230,9 +239,10 @@ def run_ours(args):
         "paper_context": "138,000 zones/s per K20 GPU, 48,000 zones/s per 16-core node (PAPER.md L414; 64^3/device)",
     }
     if world == 1 and not args.no_cpu_baseline:
-        v, sps, cores = oracle_sample(args.ref_n, 2, 0)
+        v, sps, cores = oracle_sample(args.ref_n, args.ref_steps, 0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
-                                "sample": "config-3 generator at %d^3, 2 time steps (%.1f s)" % (args.ref_n, 2 * sps)}
+                                "sample": "config-3 generator at %d^3, %d time steps (%.1f s)"
+                                          % (args.ref_n, args.ref_steps, args.ref_steps * sps)}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -244,7 +254,9 @@ def main():
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--n", type=int, default=256, help="zones per direction per GPU (headline 256)")
-    ap.add_argument("--ref-n", type=int, default=48, help="grid size of the oracle's bounded sample")
+    ap.add_argument("--ref-n", type=int, default=96, help="grid size of the oracle's bounded sample")
+    ap.add_argument("--ref-steps", type=int, default=12,
+                    help="time steps of the oracle's sample in the cpu_baseline leg (96^3 x 12 ~ 15 s on 16 cores)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
