@@ -169,6 +169,7 @@ int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, double *U);
  *          order 00 01 02 03 11 12 13 22 23 33, 10..19 = g^mu^nu (same order), 20 = sqrt(-g), 21 = lapse,
  *          22 = tau_R (used when tau_mode == GRIM_TAU_R32; otherwise the descriptor's tau)      (4*23*n2d doubles)
  *   conn : [l*16 + m*4 + n][idx2d] = Gamma^l_{mn} at zone centres                                (64*n2d doubles)
+ *          symmetric in (m, n): the kernels read the m <= n entries and use them for both orders
  * The library derives alpha g^{ti} (one multiplication per entry) and copies the rest unchanged.  Afterwards the
  * context behaves as after grim_set_metric(GRIM_KERR_MKS): general-metric kernels.  Synchronises. */
 int grim_set_metric_tables(grim_ctx *c, const double *tab, const double *conn);

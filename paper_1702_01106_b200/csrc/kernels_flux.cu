@@ -96,8 +96,11 @@ struct FaceTile {
 #ifndef GRIM_FLUX_MINB
 #define GRIM_FLUX_MINB 4
 #endif
+#ifndef GRIM_FLUX_MINB_GEN
+#define GRIM_FLUX_MINB_GEN 4
+#endif
 template <int N, int RECON, class G, int DIR>  // DIR = 0..2
-__global__ void __launch_bounds__(FB, GRIM_FLUX_MINB)
+__global__ void __launch_bounds__(FB, G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN)
 face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE, double *__restrict__ Fface,
                  double *__restrict__ cface) {
   using T = FaceTile<DIR>;
@@ -227,6 +230,22 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
   }
   sp_loc[3] = ssum;
 
+  // the zone's connection coefficients, one batch of independent loads; the three contractions below read them
+  // from registers (they were 3 x 64 loads feeding serial sums)
+  double cn[G::flat ? 1 : CONN_NCOMP];
+  if constexpr (!G::flat) {
+#pragma unroll
+    for (int l = 0; l < 4; l++)
+#pragma unroll
+      for (int m = 0; m < 4; m++)
+#pragma unroll
+        for (int n = m; n < 4; n++) {  // Gamma^l_{mn} = Gamma^l_{nm}: the tables hold both, 40 loads serve 64
+          const double c = __ldg(gv.conn + (l * 16 + m * 4 + n) * gv.n2d + id);
+          cn[l * 16 + m * 4 + n] = c;
+          cn[l * 16 + n * 4 + m] = c;
+        }
+  }
+
   // explicit geometric source sqrt(-g) T^k_l Gamma^l_{nu k} at P_E (eq 31; C-5)
   double SE[4] = {0.0, 0.0, 0.0, 0.0};
   if constexpr (!G::flat) {
@@ -241,7 +260,7 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
 #pragma unroll
       for (int kk = 0; kk < 4; kk++)
 #pragma unroll
-        for (int l = 0; l < 4; l++) s = s + T[kk][l] * gv.conn[(l * 16 + nu * 4 + kk) * gv.n2d + id];
+        for (int l = 0; l < 4; l++) s = s + T[kk][l] * cn[l * 16 + nu * 4 + kk];
       SE[nu] = gc.sqrtmg() * s;
     }
   }
@@ -320,7 +339,7 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
         for (int nu = 0; nu < 4; nu++)
 #pragma unroll
           for (int l = 0; l < 4; l++)
-            gam = gam + gv.conn[(l * 16 + nu * 4 + mu) * gv.n2d + id] * ucon[nu] * ucov[l];
+            gam = gam + cn[l * 16 + nu * 4 + mu] * ucon[nu] * ucov[l];
         acc = acc - gam;
       }
       ba = ba + bh[mu] * acc;
@@ -343,7 +362,7 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
         for (int nu = 0; nu < 4; nu++)
 #pragma unroll
           for (int l = 0; l < 4; l++)
-            gbb = gbb + gv.conn[(l * 16 + mu * 4 + nu) * gv.n2d + id] * bh[mu] * bh[nu] * ucov[l];
+            gbb = gbb + cn[l * 16 + mu * 4 + nu] * bh[mu] * bh[nu] * ucov[l];
       Xd = bbdu - gbb;
     }
     Gout[0] = bgradTh + sE.th.Th * ba;
@@ -369,8 +388,11 @@ __device__ __noinline__ void stage_const_replay(const GridView &gv, const double
 #ifndef GRIM_SC_MINB
 #define GRIM_SC_MINB 4
 #endif
+#ifndef GRIM_SC_MINB_GEN
+#define GRIM_SC_MINB_GEN 2  // general metric: connection contractions, 6 neighbour geometries -> 255 registers
+#endif
 template <int N, class G>
-__global__ void __launch_bounds__(FB, GRIM_SC_MINB)
+__global__ void __launch_bounds__(FB, G::flat ? GRIM_SC_MINB : GRIM_SC_MINB_GEN)
 stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE,
                    const double *__restrict__ Pn, double dt_stage, const double *__restrict__ Fface,
                    const double *__restrict__ cface, double *__restrict__ C, double *__restrict__ Gx,
