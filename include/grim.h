@@ -131,6 +131,15 @@ int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_E, const do
                      double dt_stage, int32_t max_iters, double *P_iter, double *resnorm, int32_t *status,
                      int32_t *iters, int64_t *n_active_out);
 
+/* Steps a4-a7 as one fresh solve (what grim_timestep enqueues per stage): every interior zone starts from
+ * P_guess with status = iters = 0 and iterates to a terminal status; the result goes to P_out (interior zones only;
+ * ghost zones of P_out are not touched).  P_out may be P_guess, and it may be P_n: a zone's inputs are read before
+ * its result is written and no other zone reads them.  resnorm, status, iters : Zg each or NULL (context scratch).
+ * Other arguments as grim_newton_step.  Does not synchronise. */
+int grim_newton_solve(grim_ctx *c, const double *P_n, const double *P_E, const double *C, const double *G,
+                      double dt_stage, const double *P_guess, double *P_out, double *resnorm, int32_t *status,
+                      int32_t *iters);
+
 /* Standalone primitive recovery (O-10; BASELINE config 2): for each of nz zones solves
  * R(P) = (U(P) - U*)/||U*||_2 = 0 by the same Newton iteration, tol = rtol.
  *   U_target : N*nz flat   geom : NULL (Minkowski) -- curved-space flat inversion is not implemented (GRIM_EINVAL)

@@ -48,6 +48,7 @@ _SIGNATURES = {
     "grim_set_metric_tables": (C.c_int, [_vp, _pd, _pd]),
     "grim_compute_fluxes": (C.c_int, [_vp, _vp, _vp, _dbl, _vp, _vp, _vp]),
     "grim_newton_step": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _i32, _vp, _vp, _vp, _vp, _pi64]),
+    "grim_newton_solve": (C.c_int, [_vp, _vp, _vp, _vp, _vp, _dbl, _vp, _vp, _vp, _vp, _vp]),
     "grim_invert_primitives": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
     "grim_timestep": (C.c_int, [_vp, _vp, _dbl, _pd, C.POINTER(StepStats)]),
     "grim_free": (None, [_vp]),
@@ -231,6 +232,13 @@ class Grid:
                                              _ptr(resnorm, t.float64), _ptr(status, t.int32), _ptr(iters, t.int32),
                                              C.byref(na) if want_active else None), "grim_newton_step")
         return na.value if want_active else None
+
+    def newton_solve(self, P_n, P_E, C_, G_, dt_stage, P_guess, P_out, resnorm=None, status=None, iters=None):
+        t = self.torch
+        self._check(self._L.grim_newton_solve(self.h, _ptr(P_n, t.float64), _ptr(P_E, t.float64), _ptr(C_, t.float64),
+                                              _ptr(G_, t.float64), dt_stage, _ptr(P_guess, t.float64),
+                                              _ptr(P_out, t.float64), _ptr(resnorm, t.float64),
+                                              _ptr(status, t.int32), _ptr(iters, t.int32)), "grim_newton_solve")
 
     def invert_primitives(self, U_target, P_inout, iters, status, resnorm):
         t = self.torch

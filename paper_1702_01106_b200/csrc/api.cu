@@ -359,6 +359,23 @@ extern "C" int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_
   return GRIM_OK;
 }
 
+extern "C" int grim_newton_solve(grim_ctx *c, const double *P_n, const double *P_E, const double *C, const double *G,
+                                 double dt_stage, const double *P_guess, double *P_out, double *resnorm,
+                                 int32_t *status, int32_t *iters) {
+  int rc = need_metric(c);
+  if (rc) return rc;
+  if (!P_n || !P_E || !P_guess || !P_out) return fail(c, GRIM_EINVAL, "grim_newton_solve: null array argument");
+  if (!(dt_stage > 0.0)) return fail(c, GRIM_EINVAL, "dt_stage must be positive");
+  CU(cudaSetDevice(c->d.device));
+  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
+  c->launches += timed(c, GRIM_K_NEWTON, [&] {
+    return launch_newton_stage(c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, P_guess, 1, dt_stage, 0, P_out,
+                               resnorm ? resnorm : c->resnorm, status ? status : c->status,
+                               iters ? iters : c->iters, c->cnt, c->stream);
+  });
+  return check_launch(c, "newton_stage kernel");
+}
+
 extern "C" int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, double *U) {
   if (!c || !P || !U || nz < 0) return fail(c, GRIM_EINVAL, "grim_prim_to_conserved: bad argument");
   CU(cudaSetDevice(c->d.device));

@@ -87,7 +87,7 @@ class SlabGrid:
             if g.ngd[2] == 0:
                 raise gb.GrimError("slab decomposition needs an active X^3 direction")
             t = torch
-            self.Ph, self.Pnew = g.zeros(g.nvar), g.zeros(g.nvar)
+            self.Ph = g.zeros(g.nvar)
             self.rn = g.zeros()
             self.st, self.it = g.zeros(dtype=t.int32), g.zeros(dtype=t.int32)
             self.sp = t.zeros(4, dtype=t.float64, device=g.device)
@@ -114,17 +114,15 @@ class SlabGrid:
         if self.world == 1:
             g.timestep(P, dt)
             return
+        # no stage-buffer copies: each solve reads its guess from P_E and writes the interior of its output; the
+        # X^3 ghost planes of P_{n+1/2} come from the neighbours, the others from the boundary conditions; the
+        # second solve writes P_{n+1} over P_n zone by zone (grim_newton_solve)
         self._ghosts(P)
         g.compute_fluxes(P, P, 0.5 * dt)
-        self.Ph.copy_(P)
-        self.st.zero_(); self.it.zero_()
-        g.newton_step(P, P, None, None, 0.5 * dt, 0, self.Ph, self.rn, self.st, self.it, want_active=False)
+        g.newton_solve(P, P, None, None, 0.5 * dt, P, self.Ph, self.rn, self.st, self.it)
         self._ghosts(self.Ph)
         g.compute_fluxes(self.Ph, P, dt)
-        self.Pnew.copy_(self.Ph)
-        self.st.zero_(); self.it.zero_()
-        g.newton_step(P, self.Ph, None, None, dt, 0, self.Pnew, self.rn, self.st, self.it, want_active=False)
-        P.copy_(self.Pnew)
+        g.newton_solve(P, self.Ph, None, None, dt, self.Ph, P, self.rn, self.st, self.it)
 
     def timestep_host(self, hP, dt):
         """End to end with a HOST (pinned) buffer: H2D, one step, D2H."""

@@ -199,3 +199,59 @@ def test_timestep_host_equals_device_path():
     hP = torch.from_numpy(P0.copy()).pin_memory()
     gc.timestep_host(hP, 2, 0.004)
     assert np.array_equal(hP.numpy(), dP.cpu().numpy())
+
+
+def test_two_slabs_equal_single_grid():
+    """The multi-GPU stage sequence (distributed.py::SlabGrid.timestep: ghost fill + X^3 plane exchange,
+    grim_compute_fluxes, grim_newton_solve; no stage-buffer copies, second solve written over P_n) on two slabs of a
+    periodic 3-D grid held on ONE device, the exchange done by plain tensor copies: each slab's result must be
+    bit-identical to its part of the single-grid grim_timestep result -- and to the oracle's."""
+    import torch
+    from paper_1702_01106_b200 import workloads
+    import paper_1702_01106_b200 as gb
+    n, ng = 12, 3
+    gk, P0 = workloads.config3(n=n)
+    go = oracle_grid(gk)
+    dt = go.choose_dt(P0)
+    ref = to_dev(P0)
+    cuda_grid(gk).timestep(ref, dt)
+    h = n // 2
+    gks = dict(gk, n3=h, xend=(1.0, 1.0, 0.5), bc=[[0, 0], [0, 0], [gb.BC_NONE, gb.BC_NONE]])
+    slabs = [cuda_grid(gks), cuda_grid(dict(gks, xstart=(0.0, 0.0, 0.5), xend=(1.0, 1.0, 1.0)))]
+    P = [to_dev(P0[:, r * h:r * h + h + 2 * ng].copy()) for r in range(2)]
+    Ph = [torch.zeros_like(p) for p in P]
+
+    def ghosts(A):
+        for r in range(2):
+            slabs[r].fill_ghosts(A[r])
+        for r in range(2):                      # periodic pair: both neighbours of slab r are slab 1-r
+            A[r][:, :ng] = A[1 - r][:, h:h + ng]
+            A[r][:, ng + h:] = A[1 - r][:, ng:2 * ng]
+
+    ghosts(P)
+    for r in range(2):
+        slabs[r].compute_fluxes(P[r], P[r], 0.5 * dt)
+        slabs[r].newton_solve(P[r], P[r], None, None, 0.5 * dt, P[r], Ph[r])
+    ghosts(Ph)
+    for r in range(2):
+        slabs[r].compute_fluxes(Ph[r], P[r], dt)
+        slabs[r].newton_solve(P[r], Ph[r], None, None, dt, Ph[r], P[r])
+    for r in range(2):
+        assert torch.equal(P[r][:, ng:ng + h, ng:-ng, ng:-ng], ref[:, ng + r * h:ng + r * h + h, ng:-ng, ng:-ng])
+    Po = P0.copy()
+    go.timestep(Po, dt)
+    assert np.array_equal(go.interior(ref.cpu().numpy()), go.interior(Po))
+
+
+def test_timestep_with_caller_ghosts():
+    """GRIM_BC_NONE sides: grim_timestep uses the caller's ghost zones for both stages (the stage buffer starts as a
+    copy of P).  Same as the oracle with BC_NONE."""
+    from paper_1702_01106_b200 import workloads
+    import paper_1702_01106_b200 as gb
+    gk, P0 = workloads.config3(n=10)
+    gk = dict(gk, bc=[[0, 0], [gb.BC_NONE, gb.BC_NONE], [0, 0]])
+    go, gc = oracle_grid(dict(gk, bc=[[og.BC_PERIODIC] * 2, [og.BC_NONE] * 2, [og.BC_PERIODIC] * 2])), cuda_grid(gk)
+    Po, dP = P0.copy(), to_dev(P0)
+    go.timestep(Po, 0.004)
+    gc.timestep(dP, 0.004)
+    assert np.array_equal(go.interior(dP.cpu().numpy()), go.interior(Po))
