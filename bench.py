@@ -115,6 +115,68 @@ def oracle_sample(n, steps, warmup):
     return n ** 3 * steps / el, el / steps, og.num_threads()
 
 
+def other_workloads(local):
+    """Secondary measurements, N = 1 only, after the headline timing (reported beside it, not bench lines):
+    BASELINE config 2 (2^24 standalone inversions, ideal MHD) and one EMHD time step on config 5's grid
+    (Kerr a = 0.9375, 256 x 256 x 128, synthetic state -- workloads.kerr_synthetic)."""
+    import torch
+    import paper_1702_01106_b200 as gb
+    from paper_1702_01106_b200 import workloads
+    out = {}
+
+    def ev():
+        return torch.cuda.Event(enable_timing=True)
+
+    nz, nvar = 1 << 24, 8
+    Ptrue, guess = workloads.config2(nz, seed=1702, nvar=nvar)
+    g = gb.Grid(8, 8, 1, dim=2, model=nvar, rtol=1e-12, kmax=30, lsmax=8, device=local)
+    dU = torch.empty((nvar, nz), dtype=torch.float64, device="cuda")
+    g.prim_to_conserved(torch.from_numpy(Ptrue).cuda(), dU)
+    dG = torch.from_numpy(guess).cuda()
+    it = torch.zeros(nz, dtype=torch.int32, device="cuda")
+    st = torch.zeros_like(it)
+    rn = torch.zeros(nz, dtype=torch.float64, device="cuda")
+    best = None
+    for _ in range(4):
+        dP = dG.clone()
+        torch.cuda.synchronize()
+        e0, e1 = ev(), ev()
+        e0.record()
+        g.invert_primitives(dU, dP, it, st, rn)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        best = ms if best is None else min(best, ms)
+    out["config2_inversion_2^24"] = {"ms": best, "solves_per_s": nz / best * 1e3,
+                                     "zone_iterations_per_s": float(it.double().sum()) / best * 1e3,
+                                     "mean_iterations": float(it.double().mean()),
+                                     "converged_fraction": float(((st & 1) != 0).double().mean())}
+    del g, dU, dG, dP, it, st, rn
+    torch.cuda.empty_cache()
+
+    gk, P = workloads.kerr_synthetic(256, 256, 128)
+    g = gb.Grid(gk["n1"], gk["n2"], gk["n3"], dim=3, xstart=gk["xstart"], xend=gk["xend"], bc=gk["bc"], model=10,
+                recon=1, tau_mode=gk["tau_mode"], rtol=gk["rtol"], kmax=gk["kmax"], lsmax=gk["lsmax"],
+                metric=gk["metric"], metric_params=gk["metric_params"], device=local)
+    dP = torch.from_numpy(P).cuda()
+    dt, _ = g.timestep(dP.clone(), 0.0, want_dt=True)
+    for _ in range(3):
+        g.timestep(dP, dt)
+    torch.cuda.synchronize()
+    e0, e1 = ev(), ev()
+    K = 5
+    e0.record()
+    for _ in range(K):
+        g.timestep(dP, dt)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / K
+    _, sst = g.timestep(dP, dt, want_stats=True)
+    out["kerr_emhd_256x256x128_synthetic"] = {"ms_per_step": ms, "zone_updates_per_s": g.zones / ms * 1e3,
+                                              "unconverged": [int(x) for x in sst.unconverged]}
+    return out
+
+
 def run_reference(args):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -243,6 +305,13 @@ def run_ours(args):
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": "config-3 generator at %d^3, %d time steps (%.1f s)"
                                           % (args.ref_n, args.ref_steps, args.ref_steps * sps)}
+    if world == 1 and not args.no_extras:
+        del dP, hP, slab, g
+        torch.cuda.empty_cache()
+        try:
+            line["other_workloads"] = other_workloads(local)
+        except Exception as e:          # secondary numbers never cost the headline line
+            line["other_workloads"] = {"error": repr(e)}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
@@ -259,6 +328,7 @@ def main():
                     help="time steps of the oracle's sample in the cpu_baseline leg (96^3 x 12 ~ 15 s on 16 cores)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads (config 2, Kerr step)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     if args.impl == "reference":

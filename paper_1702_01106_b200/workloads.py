@@ -92,3 +92,36 @@ def config2(nz, seed=1702, nvar=8):
         P[9] = 0.1 * rng.uniform(-1.0, 1.0, nz) * pg
     guess = P * (1.0 + 0.1 * xi)
     return P, guess
+
+
+def kerr_synthetic(n1=256, n2=256, n3=128, nvar=10, seed=9375, a=0.9375, h=0.3):
+    """Stand-in for BASELINE configs 4-5 (the Fishbone-Moncrief closed form is not in PAPER.md): a smooth seeded
+    EMHD state on the same grid -- Kerr a = 0.9375 in modified Kerr-Schild coordinates (h = 0.3), X^1 = ln r in
+    [ln 1.3, ln 40], X^2 in [0, 1], X^3 = phi in [0, 2 pi) (n3 = 1: 2-D), outflow / polar reflection / periodic
+    boundaries, tau_R = r^{3/2}, closure coefficients 1, MP5 -- with power-law radial profiles, a poloidal-angle
+    modulation and 0.1 % white noise.  Returns (grid description, P[nvar, s3, s2, s1]); ghosts are not filled."""
+    dim = 3 if n3 > 1 else 2
+    grid = dict(n1=n1, n2=n2, n3=n3, ng=3, dim=dim, nvar=nvar, recon=1, limiter_theta=1.0,
+                xstart=(float(np.log(1.3)), 0.0, 0.0), xend=(float(np.log(40.0)), 1.0, float(2 * np.pi)),
+                bc=[[1, 1], [2, 2], [0, 0]], tau_mode=1, metric=1, metric_params=(a, h), gam=4.0 / 3.0,
+                phi=1.0, psi=1.0, rtol=1e-12, kmax=8, lsmax=5, cfl=0.5)
+    ngd = (3, 3, 3 if dim == 3 else 0)
+    X1, X2, _ = padded_centres((n1, n2, n3), ngd, grid["xstart"], grid["xend"])
+    X1, X2 = X1[:1], X2[:1]
+    r = np.exp(X1)
+    s3 = n3 + 2 * ngd[2]
+    P = np.zeros((nvar, s3) + X1.shape[1:])
+    P[0] = r ** -1.5 * (1 + 0.1 * np.sin(3 * X1) * np.cos(2 * np.pi * X2))
+    P[1] = 0.1 * r ** -2.5 * (1 + 0.1 * np.cos(2 * X1 + 1.0))
+    P[2] = -0.05 / r * (1 + 0.2 * np.sin(2 * np.pi * X2))
+    P[3] = 0.002 * np.sin(2 * np.pi * X2) / r
+    P[4] = 0.05 * r ** -1.5
+    P[5] = 0.02 * r ** -3 * (1 + 0.3 * np.cos(np.pi * X2))
+    P[6] = 0.002 * r ** -3 * np.sin(2 * np.pi * X2)
+    P[7] = 0.01 * r ** -3
+    if nvar == 10:
+        P[8] = 1e-3 * P[0] * (P[1] / (3 * P[0])) ** 1.5 * np.sin(2 * np.pi * X2 + 0.3)
+        P[9] = 1e-2 * P[1] / 3 * np.cos(X1)
+    rng = np.random.Generator(np.random.PCG64(seed))
+    P *= 1 + 1e-3 * rng.standard_normal(P.shape)
+    return grid, P
