@@ -88,6 +88,9 @@ typedef struct {
   double cfl;               /* Courant factor (L651; C-15)                                                  */
   int32_t device;           /* CUDA device ordinal                                                          */
   void *stream;             /* cudaStream_t; NULL = the legacy default stream                               */
+  int32_t flux_ct;          /* != 0: flux-CT averaging of the B-field face fluxes between a2 and a3 (L327-335):
+                               face -> edge -> face simple averages (Toth 2000 as in harm), F^d(B^d) = 0; keeps the
+                               cell-corner-centred div B at round-off.  Needs ghost zones filled in the corners.    */
 } grim_grid_desc;
 
 typedef struct {

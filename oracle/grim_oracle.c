@@ -692,6 +692,63 @@ static void face_flux(const og_grid *g, const double *PE, int dir, int i, int j,
 }
 
 /* ===================================================================================
+ * NEXT-1  Flux-CT (section 4.2).  The paper names the scheme (Toth 2000, "also being used in
+ * the harm code", simple averaging without upwinding) and does not print it; this is that scheme:
+ *   edge (i-1/2, j-1/2, k):  E3 = [F1(B2)(i,j) + F1(B2)(i,j-1) - F2(B1)(i,j) - F2(B1)(i-1,j)] / 4
+ *   edge (i, j-1/2, k-1/2):  E1 = [F2(B3)(j,k) + F2(B3)(j,k-1) - F3(B2)(j,k) - F3(B2)(j-1,k)] / 4
+ *   edge (i-1/2, j, k-1/2):  E2 = [F3(B1)(k,i) + F3(B1)(k,i-1) - F1(B3)(k,i) - F1(B3)(k-1,i)] / 4
+ *   F1(B1) = 0, F1(B2)(i,j,k) =  [E3(i,j,k) + E3(i,j+1,k)]/2, F1(B3)(i,j,k) = -[E2(i,j,k) + E2(i,j,k+1)]/2
+ *   F2(B2) = 0, F2(B3)(i,j,k) =  [E1(i,j,k) + E1(i,j,k+1)]/2, F2(B1)(i,j,k) = -[E3(i,j,k) + E3(i+1,j,k)]/2
+ *   F3(B3) = 0, F3(B1)(i,j,k) =  [E2(i,j,k) + E2(i+1,j,k)]/2, F3(B2)(i,j,k) = -[E1(i,j,k) + E1(i,j+1,k)]/2
+ * with F^j(B^i) = sqrt(-g)(b^i u^j - b^j u^i) (eq 32, G-3), so that F1(B2) = -F2(B1) etc. are the same edge field
+ * seen from two faces.  A pair whose second direction is inactive (2-D: E1, E2) is left out and the fluxes it
+ * would replace stay as the Riemann solver gave them.
+ * =================================================================================== */
+void og_flux_ct(const og_grid *g, double *const Fface[3]) {
+  const int64_t zg = g->zg;
+  const int act[3] = {g->ngd[0] > 0, g->ngd[1] > 0, g->ngd[2] > 0};
+  int lo[3], hi[3];                      /* edges: every active index in [ng, ng+n] */
+  for (int a = 0; a < 3; a++) { lo[a] = g->ngd[a]; hi[a] = g->ngd[a] + g->n[a] + (act[a] ? 1 : 0); }
+  const int64_t st[3] = {1, g->sz[0], (int64_t)g->sz[0] * g->sz[1]};
+  double *E[3] = {NULL, NULL, NULL};
+  /* E[c]: edge field along direction c, from the fluxes of the two directions a, b = c+1, c+2 (cyclic) */
+  for (int c = 0; c < 3; c++) {
+    int a = (c + 1) % 3, b = (c + 2) % 3;
+    if (!act[a] || !act[b]) continue;
+    E[c] = (double *)calloc((size_t)zg, sizeof(double));
+    const double *Fa_Bb = Fface[a] + (int64_t)(OG_B1 + b) * zg;   /* F^a(B^b) */
+    const double *Fb_Ba = Fface[b] + (int64_t)(OG_B1 + a) * zg;   /* F^b(B^a) = -F^a(B^b) at the same point */
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = lo[2]; k < hi[2]; k++)
+      for (int j = lo[1]; j < hi[1]; j++)
+        for (int i = lo[0]; i < hi[0]; i++) {
+          int64_t z = zidx(g, i, j, k);
+          E[c][z] = 0.25 * (Fa_Bb[z] + Fa_Bb[z - st[b]] - Fb_Ba[z] - Fb_Ba[z - st[a]]);
+        }
+  }
+  /* back to the faces of the interior zones */
+  for (int a = 0; a < 3; a++) {
+    if (!act[a]) continue;
+    int b = (a + 1) % 3, c = (a + 2) % 3;   /* F^a(B^b) = +avg_b E[c];  F^a(B^c) = -avg_c E[b] */
+    double *Fa_Ba = Fface[a] + (int64_t)(OG_B1 + a) * zg;
+    double *Fa_Bb = Fface[a] + (int64_t)(OG_B1 + b) * zg;
+    double *Fa_Bc = Fface[a] + (int64_t)(OG_B1 + c) * zg;
+    int fh[3] = {g->ngd[0] + g->n[0], g->ngd[1] + g->n[1], g->ngd[2] + g->n[2]};
+    fh[a] += 1;
+#pragma omp parallel for collapse(2) schedule(static)
+    for (int k = g->ngd[2]; k < fh[2]; k++)
+      for (int j = g->ngd[1]; j < fh[1]; j++)
+        for (int i = g->ngd[0]; i < fh[0]; i++) {
+          int64_t z = zidx(g, i, j, k);
+          Fa_Ba[z] = 0.0;
+          if (E[c]) Fa_Bb[z] = 0.5 * (E[c][z] + E[c][z + st[b]]);
+          if (E[b]) Fa_Bc[z] = -(0.5 * (E[b][z] + E[b][z + st[c]]));
+        }
+  }
+  for (int c = 0; c < 3; c++) free(E[c]);
+}
+
+/* ===================================================================================
  * O-8  Stage precompute: C = -U(P_n)/dt' + divF(P_E) - S^E(P_E) and the spatial-gradient terms of
  * the EMHD sources (L438, eq 19, eq 13; C-5)
  * =================================================================================== */
@@ -706,12 +763,16 @@ void og_stage_prepare(const og_grid *g, const double *Pn, const double *PE, doub
     if (g->ngd[a] == 0) continue;
     Fface[a] = (double *)calloc((size_t)(nv * zg), sizeof(double));
     cface[a] = (double *)calloc((size_t)zg, sizeof(double));
+    int lo[3] = {g->ngd[0], g->ngd[1], g->ngd[2]};
     int hi[3] = {g->ngd[0] + g->n[0], g->ngd[1] + g->n[1], g->ngd[2] + g->n[2]};
     hi[a] += 1;
+    if (g->d.flux_ct)                     /* the edge averages reach one face into the transverse ghost zones */
+      for (int b = 0; b < 3; b++)
+        if (b != a && g->ngd[b] > 0) { lo[b] -= 1; hi[b] += 1; }
 #pragma omp parallel for collapse(2) schedule(static)
-    for (int k = g->ngd[2]; k < hi[2]; k++)
-      for (int j = g->ngd[1]; j < hi[1]; j++)
-        for (int i = g->ngd[0]; i < hi[0]; i++) {
+    for (int k = lo[2]; k < hi[2]; k++)
+      for (int j = lo[1]; j < hi[1]; j++)
+        for (int i = lo[0]; i < hi[0]; i++) {
           double F[OG_NMAX], c;
           face_flux(g, PE, a, i, j, k, F, &c);
           int64_t z = zidx(g, i, j, k);
@@ -719,6 +780,7 @@ void og_stage_prepare(const og_grid *g, const double *Pn, const double *PE, doub
           cface[a][z] = c;
         }
   }
+  if (g->d.flux_ct) og_flux_ct(g, Fface);
   double smax[4] = {0, 0, 0, 0};
 #pragma omp parallel
   {

@@ -80,6 +80,7 @@ typedef struct {
   double  fd_eps, eps_bt, atol, rtol;
   int32_t kmax, lsmax;
   double  cfl;
+  int32_t flux_ct;    /* != 0: flux-CT averaging of the magnetic-field fluxes (PAPER.md 4.2, L327-335) */
 } og_grid_desc;
 
 typedef struct {
@@ -124,6 +125,12 @@ void     og_fill_ghosts(const og_grid *g, double *P);
 void     og_grid_get_geom(const og_grid *g, int loc /*0 centre,1..3 lower faces*/, int64_t idx2d, og_geom *out);
 void     og_grid_get_conn(const og_grid *g, int64_t idx2d, double conn[4][4][4]);
 double   og_grid_get_tau(const og_grid *g, int loc, int64_t idx2d);   /* tau_R of that evaluation point (C-11) */
+/* Flux-CT (PAPER.md 4.2 L327-335: Toth 2000 as used in harm): face-centred electric fields F^j(B^i) -> simple
+   average to the edges -> average back to the faces; F^d(B^d) = 0.  Fface[a]: nvar*zg face fluxes of direction a
+   (NULL for an inactive direction), valid on faces whose index along a is in [ng, ng+n] and whose transverse
+   indices are in [ng-1, ng+n]; on return the B^i entries hold the averaged fluxes on the faces of the interior
+   zones.  The cell-corner-centred div B of Toth's scheme is then unchanged by the update to round-off. */
+void     og_flux_ct(const og_grid *g, double *const Fface[3]);
 /* stage constant C (nvar x Zg) and explicit EMHD gradient terms G (3 x Zg: Xq, Xd, divx) (L438).
    speeds[0..2] = max_z c^d/dX^d, speeds[3] = max_z sum_d c^d/dX^d */
 void     og_stage_prepare(const og_grid *g, const double *Pn, const double *PE, double dt_stage,

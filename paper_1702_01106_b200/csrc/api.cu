@@ -28,6 +28,7 @@ struct grim_ctx {
   // scratch
   double *C, *G;               // stage constant, EMHD gradient terms
   double *Fface, *cface;       // face fluxes (3 x N x Zg), face speeds (3 x Zg)
+  double *emf;                 // edge fields (3 x Zg), flux-CT only
   double *Ph, *Pnew;           // stage buffers
   double *resnorm;
   int32_t *status, *iters;
@@ -140,7 +141,7 @@ extern "C" void grim_free(grim_ctx *c) {
   cudaStreamSynchronize(c->stream);
   drain_spans(c);
   void *ptrs[] = {c->geomC, c->geomF[0], c->geomF[1], c->geomF[2], c->conn, c->C, c->G, c->Fface, c->cface,
-                  c->Ph, c->Pnew, c->resnorm, c->status, c->iters, c->cnt, c->stats, c->probe_sink,
+                  c->emf, c->Ph, c->Pnew, c->resnorm, c->status, c->iters, c->cnt, c->stats, c->probe_sink,
                   c->list[0], c->list[1], c->hostP, c->invbuf};
   for (void *p : ptrs)
     if (p) cudaFree(p);
@@ -231,6 +232,7 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   A_(c->G, 3 * zg * 8);
   A_(c->Fface, 3 * N * zg * 8);
   A_(c->cface, 3 * zg * 8);
+  if (d->flux_ct) A_(c->emf, 3 * zg * 8);
   A_(c->Ph, N * zg * 8);
   A_(c->Pnew, N * zg * 8);
   A_(c->resnorm, zg * 8);
@@ -248,6 +250,8 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   gv.geomC = c->geomC;
   for (int a = 0; a < 3; a++) gv.geomF[a] = c->geomF[a];
   gv.conn = c->conn;
+  gv.flux_ct = d->flux_ct ? 1 : 0;
+  gv.emf = c->emf;
   cudaMemsetAsync(c->G, 0, 3 * zg * 8, c->stream);
   cudaMemsetAsync(c->C, 0, N * zg * 8, c->stream);
   *out = c;

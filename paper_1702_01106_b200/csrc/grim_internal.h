@@ -34,6 +34,8 @@ struct GridView {
   const double *geomC;       // GT_NCOMP * n2d
   const double *geomF[3];    // lower faces
   const double *conn;        // CONN_NCOMP * n2d
+  int flux_ct;               // flux-CT averaging of the B-field fluxes
+  double *emf;               // 3 * zg edge fields (flux_ct only)
 };
 
 // per-call device counters

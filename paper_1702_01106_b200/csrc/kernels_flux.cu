@@ -151,19 +151,22 @@ face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__
   }
 }
 
-// The upper boundary faces of direction DIR (face index n along DIR): one thread per face, stencil read
-// directly from the grid array.  1/n of the faces.
+// Faces of direction DIR in a box of padded coordinates [lo, lo + cnt): one thread per face, stencil read directly
+// from the grid array.  Used for what the tiles do not cover: the upper boundary faces (face index n along DIR),
+// and with flux-CT the faces one zone into the transverse ghost layers.
+struct FaceBox {
+  int lo[3], cnt[3];
+};
 template <int N, int RECON, class G, int DIR>
-__global__ void __launch_bounds__(FB, GRIM_FLUX_MINB)
-face_edge_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE, double *__restrict__ Fface,
-                 double *__restrict__ cface) {
-  const int na = (DIR == 0) ? gv.n[1] : gv.n[0], nb = (DIR == 2) ? gv.n[1] : gv.n[2];  // the plane's extents
+__global__ void __launch_bounds__(FB, G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN)
+face_box_kernel(const __grid_constant__ GridView gv, const __grid_constant__ FaceBox bx,
+                const double *__restrict__ PE, double *__restrict__ Fface, double *__restrict__ cface) {
   const long long t = (long long)blockIdx.x * FB + threadIdx.x;
-  if (t >= (long long)na * nb) return;
-  const int ta = (int)(t % na), tb = (int)(t / na);
-  const int i = (DIR == 0) ? gv.ngd[0] + gv.n[0] : gv.ngd[0] + ta;
-  const int j = (DIR == 0) ? gv.ngd[1] + ta : (DIR == 1) ? gv.ngd[1] + gv.n[1] : gv.ngd[1] + tb;
-  const int k = (DIR == 2) ? gv.ngd[2] + gv.n[2] : gv.ngd[2] + tb;
+  if (t >= (long long)bx.cnt[0] * bx.cnt[1] * bx.cnt[2]) return;
+  const int i = bx.lo[0] + (int)(t % bx.cnt[0]);
+  const long long r = t / bx.cnt[0];
+  const int j = bx.lo[1] + (int)(r % bx.cnt[1]);
+  const int k = bx.lo[2] + (int)(r / bx.cnt[1]);
   const long long z = zone_index(gv, i, j, k);
   const long long stride = (DIR == 0) ? 1 : (DIR == 1) ? (long long)gv.sz[0] : (long long)gv.sz[0] * gv.sz[1];
   SpecArith ar;
@@ -179,12 +182,55 @@ face_edge_kernel(const __grid_constant__ GridView gv, const double *__restrict__
   }
 }
 
+// Flux-CT, face -> edge (PAPER.md 4.2 L327-335; Toth 2000 as in harm): the edge field along direction c is the
+// simple average of the four face fluxes that represent it, E_c = [F^a(B^b)(z) + F^a(B^b)(z - e_b) - F^b(B^a)(z)
+// - F^b(B^a)(z - e_a)] / 4 with (a, b, c) cyclic; one thread per edge index in [ng, ng + n] of every active
+// direction.  Pairs with an inactive direction are left out.
+template <int N>
+__global__ void __launch_bounds__(256)
+emf_kernel(const __grid_constant__ GridView gv, const double *__restrict__ Fface, double *__restrict__ emf) {
+  const int c0 = gv.n[0] + (gv.ngd[0] > 0), c1 = gv.n[1] + (gv.ngd[1] > 0), c2 = gv.n[2] + (gv.ngd[2] > 0);
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= (long long)c0 * c1 * c2) return;
+  const int i = gv.ngd[0] + (int)(t % c0);
+  const long long r = t / c0;
+  const int j = gv.ngd[1] + (int)(r % c1), k = gv.ngd[2] + (int)(r / c1);
+  const long long z = zone_index(gv, i, j, k);
+  const long long st[3] = {1, (long long)gv.sz[0], (long long)gv.sz[0] * gv.sz[1]};
+#pragma unroll
+  for (int c = 0; c < 3; c++) {
+    const int a = (c + 1) % 3, b = (c + 2) % 3;
+    if (gv.ngd[a] == 0 || gv.ngd[b] == 0) continue;
+    const double *Fa_Bb = Fface + ((long long)a * N + B1 + b) * gv.zg;
+    const double *Fb_Ba = Fface + ((long long)b * N + B1 + a) * gv.zg;
+    emf[c * gv.zg + z] = 0.25 * (Fa_Bb[z] + Fa_Bb[z - st[b]] - Fb_Ba[z] - Fb_Ba[z - st[a]]);
+  }
+}
+
+// Flux-CT, edge -> face: the flux of B^comp (comp = 0..2) through the lower a-face of zone z.  F^a(B^a) = 0,
+// F^a(B^b) = [E_c(z) + E_c(z + e_b)] / 2, F^a(B^c) = -[E_b(z) + E_b(z + e_c)] / 2, (a, b, c) cyclic; where the
+// edge field does not exist (inactive direction) the Riemann solver's flux stays.
+template <int N>
+__device__ __forceinline__ double ct_face_flux(const GridView &gv, const double *__restrict__ Fface, int a, int comp,
+                                               long long z, const long long (&st)[3]) {
+  const int b = (a + 1) % 3, c = (a + 2) % 3;
+  if (comp == a) return 0.0;
+  if (comp == b) {
+    if (gv.ngd[b] == 0) return Fface[((long long)a * N + B1 + comp) * gv.zg + z];
+    const double *E = gv.emf + c * gv.zg;
+    return 0.5 * (E[z] + E[z + st[b]]);
+  }
+  if (gv.ngd[c] == 0) return Fface[((long long)a * N + B1 + comp) * gv.zg + z];
+  const double *E = gv.emf + b * gv.zg;
+  return -(0.5 * (E[z] + E[z + st[c]]));
+}
+
 __device__ __forceinline__ void atomic_max_nonneg(unsigned long long *addr, double v) {
   atomicMax(addr, (unsigned long long)__double_as_longlong(v));
 }
 
 // Stage constant, EMHD gradient terms and wave-speed figures of padded zone z under arithmetic policy A
-template <int N, class G, class A>
+template <int N, class G, bool CT, class A>
 __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, const double *__restrict__ PE,
                                                     const double *__restrict__ Pn, double dt_stage,
                                                     const double *__restrict__ Fface,
@@ -221,7 +267,15 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
     const double *ca = cface + (long long)a * gv.zg;
     const long long zu = z + strides[a];
 #pragma unroll
-    for (int v = 0; v < N; v++) divF[v] = divF[v] + (Fa[v * gv.zg + zu] - Fa[v * gv.zg + z]) * gv.idx[a];
+    for (int v = 0; v < N; v++) {
+      if (CT && v >= B1 && v <= B3) {  // flux-CT: the B-field fluxes are the edge averages
+        const double fu = ct_face_flux<N>(gv, Fface, a, v - B1, zu, strides);
+        const double fl = ct_face_flux<N>(gv, Fface, a, v - B1, z, strides);
+        divF[v] = divF[v] + (fu - fl) * gv.idx[a];
+      } else {
+        divF[v] = divF[v] + (Fa[v * gv.zg + zu] - Fa[v * gv.zg + z]) * gv.idx[a];
+      }
+    }
     if (want_speeds) {  // only the dt probe needs them (C-15)
       const double cz = fmax(ca[z], ca[zu]) * gv.idx[a];
       sp_loc[a] = cz;
@@ -371,7 +425,7 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
   }
 }
 
-template <int N, class G>
+template <int N, class G, bool CT>
 __device__ __noinline__ void stage_const_replay(const GridView &gv, const double *__restrict__ PE,
                                                 const double *__restrict__ Pn, double dt_stage,
                                                 const double *__restrict__ Fface, const double *__restrict__ cface,
@@ -379,7 +433,7 @@ __device__ __noinline__ void stage_const_replay(const GridView &gv, const double
                                                 double *Gout, double *sp_loc) {
   ExactArith ar;
   double C_[N], G_[3] = {0.0, 0.0, 0.0}, s_[4] = {0.0, 0.0, 0.0, 0.0};
-  stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, want_speeds, z, id, C_, G_, s_);
+  stage_const_compute<N, G, CT>(ar, gv, PE, Pn, dt_stage, Fface, cface, want_speeds, z, id, C_, G_, s_);
   for (int v = 0; v < N; v++) Cout[v] = C_[v];
   for (int v = 0; v < 3; v++) Gout[v] = G_[v];
   for (int v = 0; v < 4; v++) sp_loc[v] = s_[v];
@@ -391,7 +445,7 @@ __device__ __noinline__ void stage_const_replay(const GridView &gv, const double
 #ifndef GRIM_SC_MINB_GEN
 #define GRIM_SC_MINB_GEN 2  // general metric: connection contractions, 6 neighbour geometries -> 255 registers
 #endif
-template <int N, class G>
+template <int N, class G, bool CT>
 __global__ void __launch_bounds__(FB, G::flat ? GRIM_SC_MINB : GRIM_SC_MINB_GEN)
 stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE,
                    const double *__restrict__ Pn, double dt_stage, const double *__restrict__ Fface,
@@ -406,9 +460,9 @@ stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict
     const long long id = (long long)j * gv.sz[0] + i;
     double Cout[N], Gout[3] = {0.0, 0.0, 0.0};
     SpecArith ar;
-    stage_const_compute<N, G>(ar, gv, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
+    stage_const_compute<N, G, CT>(ar, gv, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
     if (!ar.good())
-      stage_const_replay<N, G>(gv, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
+      stage_const_replay<N, G, CT>(gv, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
 #pragma unroll
     for (int v = 0; v < N; v++) C[v * gv.zg + z] = Cout[v];
     if constexpr (N == 10) {
@@ -443,15 +497,55 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
     if (a == 0) face_flux_kernel<N, RECON, G, 0><<<tiles(128, 1, 1), FB, 0, s>>>(gv, PE, Fa, ca);
     if (a == 1) face_flux_kernel<N, RECON, G, 1><<<tiles(32, 4, 1), FB, 0, s>>>(gv, PE, Fa, ca);
     if (a == 2) face_flux_kernel<N, RECON, G, 2><<<tiles(32, 1, 4), FB, 0, s>>>(gv, PE, Fa, ca);
-    const long long ne = (long long)f0 * f1 * f2 / gv.n[a];
-    const unsigned eb = (unsigned)((ne + FB - 1) / FB);
-    if (a == 0) face_edge_kernel<N, RECON, G, 0><<<eb, FB, 0, s>>>(gv, PE, Fa, ca);
-    if (a == 1) face_edge_kernel<N, RECON, G, 1><<<eb, FB, 0, s>>>(gv, PE, Fa, ca);
-    if (a == 2) face_edge_kernel<N, RECON, G, 2><<<eb, FB, 0, s>>>(gv, PE, Fa, ca);
-    launches += 2;
+    // what the tiles leave: the upper boundary plane along a, and with flux-CT one layer of faces in every active
+    // transverse ghost direction (the edge averages reach there)
+    auto box = [&](const FaceBox &bx) {
+      const long long nf = (long long)bx.cnt[0] * bx.cnt[1] * bx.cnt[2];
+      if (nf <= 0) return;
+      const unsigned nb = (unsigned)((nf + FB - 1) / FB);
+      if (a == 0) face_box_kernel<N, RECON, G, 0><<<nb, FB, 0, s>>>(gv, bx, PE, Fa, ca);
+      if (a == 1) face_box_kernel<N, RECON, G, 1><<<nb, FB, 0, s>>>(gv, bx, PE, Fa, ca);
+      if (a == 2) face_box_kernel<N, RECON, G, 2><<<nb, FB, 0, s>>>(gv, bx, PE, Fa, ca);
+      launches++;
+    };
+    const int ext = gv.flux_ct ? 1 : 0;
+    FaceBox edge;
+    for (int d = 0; d < 3; d++) {
+      const int e = (d != a && gv.ngd[d] > 0) ? ext : 0;
+      edge.lo[d] = gv.ngd[d] - e;
+      edge.cnt[d] = gv.n[d] + 2 * e;
+    }
+    edge.lo[a] = gv.ngd[a] + gv.n[a];
+    edge.cnt[a] = 1;
+    box(edge);
+    if (ext) {
+      bool first = true;  // the first transverse direction takes the corners shared with the second
+      for (int b = 0; b < 3; b++) {
+        if (b == a || gv.ngd[b] == 0) continue;
+        for (int side = 0; side < 2; side++) {
+          FaceBox fr;
+          for (int d = 0; d < 3; d++) {
+            const int e = (d != a && d != b && gv.ngd[d] > 0 && first) ? 1 : 0;
+            fr.lo[d] = gv.ngd[d] - e;
+            fr.cnt[d] = gv.n[d] + 2 * e;
+          }
+          fr.lo[b] = side ? gv.ngd[b] + gv.n[b] : gv.ngd[b] - 1;
+          fr.cnt[b] = 1;
+          box(fr);
+        }
+        first = false;
+      }
+    }
+    launches++;
+  }
+  if (gv.flux_ct) {
+    const long long ne = (long long)(gv.n[0] + (gv.ngd[0] > 0)) * (gv.n[1] + (gv.ngd[1] > 0)) * (gv.n[2] + (gv.ngd[2] > 0));
+    emf_kernel<N><<<(unsigned)((ne + 255) / 256), 256, 0, s>>>(gv, Fface, gv.emf);
+    launches++;
   }
   const unsigned blocks = (unsigned)((gv.nint + FB - 1) / FB);
-  stage_const_kernel<N, G><<<blocks, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx, cnt);
+  if (gv.flux_ct) stage_const_kernel<N, G, true><<<blocks, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx, cnt);
+  else stage_const_kernel<N, G, false><<<blocks, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx, cnt);
   return launches + 1;
 }
 

@@ -14,7 +14,8 @@ def oracle_grid(gk, **over):
                    tau_mode=k.get("tau_mode", 0), tau=k.get("tau", 1.0), fd_eps=k.get("fd_eps", 4e-8),
                    eps_bt=k.get("eps_bt", 1e-4), atol=k.get("atol", 0.0), rtol=k.get("rtol", 1e-14),
                    kmax=k.get("kmax", 8), lsmax=k.get("lsmax", 5), cfl=k.get("cfl", 0.5),
-                   metric=k.get("metric", 0), metric_params=k.get("metric_params", ()))
+                   metric=k.get("metric", 0), metric_params=k.get("metric_params", ()),
+                   flux_ct=k.get("flux_ct", False))
 
 
 def cuda_grid(gk, **over):
@@ -28,7 +29,8 @@ def cuda_grid(gk, **over):
                    tau_mode=k.get("tau_mode", 0), tau=k.get("tau", 1.0), fd_eps=k.get("fd_eps", 4e-8),
                    eps_bt=k.get("eps_bt", 1e-4), atol=k.get("atol", 0.0), rtol=k.get("rtol", 1e-14),
                    kmax=k.get("kmax", 8), lsmax=k.get("lsmax", 5), cfl=k.get("cfl", 0.5),
-                   metric=k.get("metric", 0), metric_params=k.get("metric_params", ()))
+                   metric=k.get("metric", 0), metric_params=k.get("metric_params", ()),
+                   flux_ct=k.get("flux_ct", False))
 
 
 def to_dev(a, dtype=None):
