@@ -80,7 +80,8 @@ class SlabGrid:
                             tau=k.get("tau", 1.0), fd_eps=k.get("fd_eps", 4e-8), eps_bt=k.get("eps_bt", 1e-4),
                             atol=k.get("atol", 0.0), rtol=k.get("rtol", 1e-14), kmax=k.get("kmax", 8),
                             lsmax=k.get("lsmax", 5), cfl=k.get("cfl", 0.5), metric=k.get("metric", 0),
-                            metric_params=k.get("metric_params", ()), device=device)
+                            metric_params=k.get("metric_params", ()), device=device,
+                            flux_ct=k.get("flux_ct", False))
         self.cfl = k.get("cfl", 0.5)
         g = self.grid
         if world > 1:
