@@ -1027,6 +1027,26 @@ static double newton_zone(int n, const og_solver *sv, resid_fn fn, const void *c
 
 static void resid_stage(const void *ctx, const double *P, double *R) { zone_residual((const zone_ctx *)ctx, P, R); }
 
+/* NEXT-2  Reduced solve (L148, L643): the induction equation has no implicit source, so
+ *   sqrt(-g) B^i_new = sqrt(-g) B^i_n - dt' [div F(P_E)]_{B^i}   <=>   B^i_new = -(C_{B^i} dt') / sqrt(-g)
+ * is explicit (C = -U(P_n)/dt' + div F), and Newton runs on the M = nvar - 3 unknowns rho, u, u~^i (, q, dP) with the
+ * rows of the same equations; unknown s is primitive s for s < 5, s + 3 beyond. */
+typedef struct {
+  const zone_ctx *zc;
+  int nv;
+  double B[3];
+} reduced_ctx;
+static int reduced_prim(int s) { return s < 5 ? s : s + 3; }
+static void resid_reduced(const void *ctx, const double *X, double *R) {
+  const reduced_ctx *rc = (const reduced_ctx *)ctx;
+  double P[OG_NMAX] = {0}, Rf[OG_NMAX];
+  int M = rc->nv - 3;
+  for (int s = 0; s < M; s++) P[reduced_prim(s)] = X[s];
+  for (int d = 0; d < 3; d++) P[OG_B1 + d] = rc->B[d];
+  zone_residual(rc->zc, P, Rf);
+  for (int s = 0; s < M; s++) R[s] = Rf[reduced_prim(s)];
+}
+
 int64_t og_newton(const og_grid *g, const double *Pn, const double *PE, const double *C, const double *G,
                   double dt_stage, double *P_iter, int max_iters_this_call, double *resnorm, int32_t *status,
                   int32_t *iters, int64_t *backtracks) {
@@ -1044,8 +1064,24 @@ int64_t og_newton(const og_grid *g, const double *Pn, const double *PE, const do
         load_prims(g, P_iter, z, P);
         double tol = g->s.atol + g->s.rtol * zc.scale;
         int64_t bt = 0;
-        double rn = newton_zone(nv, &g->s, resid_stage, &zc, tol, P, &iters[z], &status[z],
-                                max_iters_this_call, &bt);
+        double rn;
+        if (g->d.reduced) {
+          reduced_ctx rc;
+          rc.zc = &zc;
+          rc.nv = nv;
+          double sg = g->geomC[(int64_t)j * g->sz[0] + i].sqrtmg;
+          for (int d = 0; d < 3; d++) {
+            rc.B[d] = -(C[(int64_t)(OG_B1 + d) * g->zg + z] * dt_stage) / sg;
+            P[OG_B1 + d] = rc.B[d];
+          }
+          double X[OG_NMAX];
+          for (int s = 0; s < nv - 3; s++) X[s] = P[reduced_prim(s)];
+          rn = newton_zone(nv - 3, &g->s, resid_reduced, &rc, tol, X, &iters[z], &status[z], max_iters_this_call,
+                           &bt);
+          for (int s = 0; s < nv - 3; s++) P[reduced_prim(s)] = X[s];
+        } else {
+          rn = newton_zone(nv, &g->s, resid_stage, &zc, tol, P, &iters[z], &status[z], max_iters_this_call, &bt);
+        }
         for (int v = 0; v < nv; v++) P_iter[(int64_t)v * g->zg + z] = P[v];
         resnorm[z] = rn;
         nbt += bt;

@@ -83,6 +83,9 @@ typedef struct {
   int32_t kmax, lsmax;
   double  cfl;
   int32_t flux_ct;    /* != 0: flux-CT averaging of the magnetic-field fluxes (PAPER.md 4.2, L327-335) */
+  int32_t reduced;    /* != 0: the paper's own split (L148 "equations without implicitly coupled source terms are
+                         treated explicitly", L643 "5 x 5 ... as opposed to a 7 x 7 Jacobian"): B^i advanced
+                         explicitly, Newton on the nvar-3 other primitives */
 } og_grid_desc;
 
 typedef struct {

@@ -43,7 +43,7 @@ class GridDesc(C.Structure):
                 ("riemann", C.c_int32), ("gam", C.c_double), ("phi", C.c_double), ("psi", C.c_double),
                 ("tau_mode", C.c_int32), ("tau", C.c_double),
                 ("fd_eps", C.c_double), ("eps_bt", C.c_double), ("atol", C.c_double), ("rtol", C.c_double),
-                ("kmax", C.c_int32), ("lsmax", C.c_int32), ("cfl", C.c_double), ("flux_ct", C.c_int32)]
+                ("kmax", C.c_int32), ("lsmax", C.c_int32), ("cfl", C.c_double), ("flux_ct", C.c_int32), ("reduced", C.c_int32)]
 
 
 class StepStats(C.Structure):
@@ -281,9 +281,10 @@ class Grid:
     def __init__(self, n1, n2=1, n3=1, ng=3, dim=2, xstart=(0, 0, 0), xend=(1, 1, 1),
                  bc=BC_PERIODIC, nvar=10, recon=MINMOD, limiter_theta=1.0, gam=4.0 / 3.0, phi=1.0, psi=1.0,
                  tau_mode=TAU_CONST, tau=1.0, fd_eps=4e-8, eps_bt=1e-4, atol=0.0, rtol=1e-14, kmax=8,
-                 lsmax=5, cfl=0.5, metric=MINKOWSKI, metric_params=(), flux_ct=False):
+                 lsmax=5, cfl=0.5, metric=MINKOWSKI, metric_params=(), flux_ct=False, reduced=False):
         d = GridDesc()
         d.flux_ct = 1 if flux_ct else 0
+        d.reduced = 1 if reduced else 0
         d.n1, d.n2, d.n3, d.ng, d.dim = n1, n2, n3, ng, dim
         for a in range(3):
             d.xstart[a], d.xend[a] = float(xstart[a]), float(xend[a])
