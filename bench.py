@@ -216,6 +216,7 @@ def run_ours(args):
     n = args.n
     gk, P0 = workloads.config3(n=n, ranks=world, rank=rank)
     gk["flux_ct"] = bool(args.flux_ct)
+    gk["reduced"] = bool(args.reduced)
     slab = gdist.SlabGrid(gk, world, rank, device=local)
     g = slab.grid
     dP = torch.from_numpy(P0).cuda()
@@ -279,7 +280,7 @@ def run_ours(args):
         "metric": METRIC, "value": zones * world * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config3-emhd-mp5-llf-minkowski-%d^3%s" % (n, "-fluxct" if args.flux_ct else ""),
+        "config": {"workload": "config3-emhd-mp5-llf-minkowski-%d^3%s" % (n, ("-fluxct" if args.flux_ct else "") + ("-reduced7" if args.reduced else "")),
                    "zones_per_gpu": zones,
                    "update": "one zone advanced one grim_timestep = 2 stages x (ghosts, MP5+LLF fluxes, stage "
                              "constants, fused Newton solve)", "dt": "fixed: CFL 0.5 on the initial data",
@@ -331,6 +332,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--flux-ct", action="store_true", help="flux-CT averaging of the B-field fluxes (not the headline)")
+    ap.add_argument("--reduced", action="store_true",
+                    help="the paper's reduced solve (B explicit, 7 x 7 Jacobian) instead of BASELINE's 10 unknowns")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads (config 2, Kerr step)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)

@@ -91,6 +91,11 @@ typedef struct {
   int32_t flux_ct;          /* != 0: flux-CT averaging of the B-field face fluxes between a2 and a3 (L327-335):
                                face -> edge -> face simple averages (Toth 2000 as in harm), F^d(B^d) = 0; keeps the
                                cell-corner-centred div B at round-off.  Needs ghost zones filled in the corners.    */
+  int32_t reduced_solve;    /* != 0: the paper's own split (L148, L643): B^i is advanced explicitly,
+                               sqrt(-g) B^i_new = sqrt(-g) B^i_n - dt' [div F]_{B^i}, and the Newton iteration of
+                               grim_newton_step / grim_newton_solve / grim_timestep runs on the other N - 3 primitives
+                               (5 x 5 / 7 x 7 Jacobian); ||R||, the tolerance and the status refer to those rows.
+                               0 (default): all N primitives are unknowns (BASELINE.json).                           */
 } grim_grid_desc;
 
 typedef struct {

@@ -35,6 +35,7 @@ struct GridView {
   const double *geomF[3];    // lower faces
   const double *conn;        // CONN_NCOMP * n2d
   int flux_ct;               // flux-CT averaging of the B-field fluxes
+  int reduced;               // reduced solve: B^i explicit, Newton on the other N - 3 primitives
   double *emf;               // 3 * zg edge fields (flux_ct only)
 };
 

@@ -25,12 +25,13 @@ struct StageArgs {
 // One zone of one stage under arithmetic policy A: loads, set-up, Newton iteration, stores.  Returns false
 // WITHOUT storing when a speculative operation saw an operand outside its safe range (fp64ops.cuh); the caller
 // then replays the zone with ExactArith.  Otherwise packs (rejected line-search trials << 1) | still-active.
-template <int N, class G, class A>
+template <int N, class G, bool RED, class A>
 __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const StageArgs &a, long long z, int i, int j,
                                           int st, double *sj) {
+  constexpr int M = Unknowns<N, RED>::M;
   StageProblem<N, G, NB> prob;
   prob.m = gv.m;
-  prob.Cs = sj + N * N * NB;
+  prob.Cs = sj + M * M * NB;
   if constexpr (G::flat) {
     prob.tau_ = gv.tau_const;
   } else {
@@ -44,7 +45,17 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
       Pn_z[v] = a.Pn[v * gv.zg + z];
       PE_z[v] = a.PE[v * gv.zg + z];
       P[v] = a.Pguess[v * gv.zg + z];
-      sj[(N * N + v) * NB] = a.C[v * gv.zg + z];
+      sj[(M * M + v) * NB] = a.C[v * gv.zg + z];
+    }
+    if constexpr (RED) {
+      // reduced solve (L148): the induction equation has no implicit source, so B^i_new = -(C_B dt') / sqrt(-g)
+      // is explicit; it stays fixed during the iteration
+#pragma unroll
+      for (int d = 0; d < 3; d++) {
+        const double b = -(prob.Cs[(B1 + d) * NB] * a.dt_stage);
+        if constexpr (G::flat) P[B1 + d] = b;
+        else P[B1 + d] = ar.div_z(b, prob.g.sqrtmg());
+      }
     }
     if constexpr (N == 10) {
       prob.Xq = a.Gx[0 * gv.zg + z];
@@ -56,8 +67,8 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
   const double tol = gv.sp.atol + gv.sp.rtol * prob.scale;
   int it = a.fresh ? 0 : a.iters[z];
   int nbt = 0;
-  JacView<N, NB> jac{sj};
-  double rn = newton_zone<N, NB>(ar, prob, gv.sp, tol, P, it, st, a.max_iters, jac, nbt);
+  JacView<M, NB> jac{sj};
+  double rn = newton_zone<N, RED, NB>(ar, prob, gv.sp, tol, P, it, st, a.max_iters, jac, nbt);
   if (!ar.good()) return -1;
 #pragma unroll
   for (int v = 0; v < N; v++) a.Piter[v * gv.zg + z] = P[v];
@@ -67,15 +78,18 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
   return (nbt << 1) | ((st & ST_TERMINAL) ? 0 : 1);
 }
 
-template <int N, class G>
+template <int N, class G, bool RED>
 __device__ __noinline__ int stage_zone_replay(const GridView &gv, const StageArgs &a, long long z, int i, int j,
                                               int st, double *sj) {
   ExactArith ar;
-  return stage_zone<N, G>(ar, gv, a, z, i, j, st, sj);
+  return stage_zone<N, G, RED>(ar, gv, a, z, i, j, st, sj);
 }
 
-template <int N, class G>
-__global__ void __launch_bounds__(NB, 256 / NB)
+#ifndef GRIM_RED_MINB
+#define GRIM_RED_MINB 2  // reduced solve: (N-3)^2 + N doubles of shared memory per zone leave room for 3 blocks
+#endif
+template <int N, class G, bool RED>
+__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : 256 / NB)
 newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
@@ -87,8 +101,8 @@ newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__
     const int st = a.fresh ? 0 : a.status[z];
     if (!(st & ST_TERMINAL)) {
       SpecArith ar;
-      res = stage_zone<N, G>(ar, gv, a, z, i, j, st, smem + threadIdx.x);
-      if (res < 0) res = stage_zone_replay<N, G>(gv, a, z, i, j, st, smem + threadIdx.x);
+      res = stage_zone<N, G, RED>(ar, gv, a, z, i, j, st, smem + threadIdx.x);
+      if (res < 0) res = stage_zone_replay<N, G, RED>(gv, a, z, i, j, st, smem + threadIdx.x);
     }
   }
   // warp-aggregated counters
@@ -100,19 +114,20 @@ newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__
   }
 }
 
-template <int N, class G>
+template <int N, class G, bool RED>
 static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *Gx,
                           const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
                           int32_t *iters, Counters *cnt, cudaStream_t s) {
-  const size_t smem = (size_t)(N * N + N) * NB * sizeof(double);  // Jacobian + C (or U*) per thread
+  constexpr int M = Unknowns<N, RED>::M;
+  const size_t smem = (size_t)(M * M + N) * NB * sizeof(double);  // Jacobian + C per thread
   static bool attr_set = false;
   if (!attr_set) {
-    cudaFuncSetAttribute(newton_stage_kernel<N, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaFuncSetAttribute(newton_stage_kernel<N, G, RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     attr_set = true;
   }
   const long long blocks = (gv.nint + NB - 1) / NB;
   const StageArgs a{Pn, PE, C, Gx, Pguess, dt_stage, max_iters, fresh, Piter, resnorm, status, iters};
-  newton_stage_kernel<N, G><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
+  newton_stage_kernel<N, G, RED><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
   return 1;
 }
 
@@ -120,12 +135,15 @@ int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, 
                         const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
                         int32_t *iters, Counters *cnt, cudaStream_t s) {
   const bool flat = (gv.metric == 0);
-  if (gv.nvar == 10) {
-    return flat ? launch_stage_t<10, GeomFlat>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
-                : launch_stage_t<10, GeomGen>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
+#define GRIM_STAGE(NV, GG, RR) \
+  launch_stage_t<NV, GG, RR>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
+  if (gv.reduced) {
+    if (gv.nvar == 10) return flat ? GRIM_STAGE(10, GeomFlat, true) : GRIM_STAGE(10, GeomGen, true);
+    return flat ? GRIM_STAGE(8, GeomFlat, true) : GRIM_STAGE(8, GeomGen, true);
   }
-  return flat ? launch_stage_t<8, GeomFlat>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
-              : launch_stage_t<8, GeomGen>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s);
+  if (gv.nvar == 10) return flat ? GRIM_STAGE(10, GeomFlat, false) : GRIM_STAGE(10, GeomGen, false);
+  return flat ? GRIM_STAGE(8, GeomFlat, false) : GRIM_STAGE(8, GeomGen, false);
+#undef GRIM_STAGE
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -162,7 +180,7 @@ __device__ __forceinline__ int invert_zone(A &ar, const GridView &gv, const Inve
   int st = a.first ? 0 : a.status[z];
   int nbt = 0;
   JacView<N, NB> jac{sj};
-  double rn = newton_zone<N, NB>(ar, prob, gv.sp, gv.sp.rtol, P, it, st, a.max_iters, jac, nbt);
+  double rn = newton_zone<N, false, NB>(ar, prob, gv.sp, gv.sp.rtol, P, it, st, a.max_iters, jac, nbt);
   if (!ar.good()) return -1;
 #pragma unroll
   for (int v = 0; v < N; v++) a.Pio[v * a.nz + z] = P[v];

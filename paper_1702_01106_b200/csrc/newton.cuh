@@ -41,6 +41,24 @@ __device__ __forceinline__ double norm2sq(const double (&R)[N]) {
   return s;
 }
 
+// The unknowns of the Newton iteration.  Full solve: all N primitives (BASELINE; C-1).  Reduced solve (RED; the
+// paper's own split, L148 / L643): B^i is advanced explicitly by the caller and stays fixed, the M = N - 3 unknowns
+// are rho, u, u~^i (, q, dP) and the residual rows are those of the same equations; unknown s is primitive prim(s).
+template <int N, bool RED>
+struct Unknowns {
+  static constexpr int M = RED ? N - 3 : N;
+  static __host__ __device__ constexpr int prim(int s) { return (!RED || s < B1) ? s : s + 3; }
+};
+
+template <int N, bool RED>
+__device__ __forceinline__ double norm2sq_rows(const double (&R)[N]) {
+  using U = Unknowns<N, RED>;
+  double s = R[U::prim(0)] * R[U::prim(0)];
+#pragma unroll
+  for (int v = 1; v < U::M; v++) s = s + R[U::prim(v)] * R[U::prim(v)];
+  return s;
+}
+
 // Residual at P with every piece recomputed; the pieces are returned for reuse.
 template <int N, class A, class Prob>
 __device__ __forceinline__ void eval_full(A &ar, const Prob &prob, const double (&P)[N], Pieces &pc, double (&R)[N]) {
@@ -81,10 +99,13 @@ struct JacView {
 };
 
 // One finite-difference column (eqs 22-23): J[:,j] = (R(P_eps,j) - R0) / (P_eps,j - P_j)
-template <int J, int N, int BLOCK, class A, class Prob>
+// (column S of the M x M Jacobian: unknown S = primitive prim(S))
+template <int S, int N, bool RED, int BLOCK, class A, class Prob>
 __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverParams &sp, const double (&P)[N],
-                                          const Pieces &base, const double (&R0)[N], const JacView<N, BLOCK> &jac,
-                                          bool &singular) {
+                                          const Pieces &base, const double (&R0)[N],
+                                          const JacView<Unknowns<N, RED>::M, BLOCK> &jac, bool &singular) {
+  using U = Unknowns<N, RED>;
+  constexpr int J = U::prim(S);
   double pj = (fabs(P[J]) < 5.0 * sp.fd_eps) ? sp.fd_eps : (1.0 + sp.fd_eps) * P[J];
   double h = pj - P[J];
   if (h == 0.0) singular = true;
@@ -92,7 +113,8 @@ __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverP
   double Rt[N];
   eval_column<J, N>(ar, prob, P, pj, base, Rt);
 #pragma unroll
-  for (int i = 0; i < N; i++) jac.at(JacView<N, BLOCK>::row(i), J) = (Rt[i] - R0[i]) * ih;
+  for (int i = 0; i < U::M; i++)
+    jac.at(JacView<U::M, BLOCK>::row(i), S) = (Rt[U::prim(i)] - R0[U::prim(i)]) * ih;
 }
 
 // Order in which the (independent) columns are evaluated: first those that reuse every piece of the unperturbed
@@ -102,8 +124,12 @@ __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverP
 #ifndef GRIM_FD_ORDER
 #define GRIM_FD_ORDER 1
 #endif
-template <int N>
+template <int N, bool RED>
 __host__ __device__ constexpr int fd_order(int s) {
+  if (RED) {  // unknown indices: rho u u~1 u~2 u~3 (q dP)
+    constexpr int red10[7] = {5, 6, 0, 1, 2, 3, 4};
+    return N == 10 ? red10[s] : s;
+  }
 #if GRIM_FD_ORDER == 1
   constexpr int ord10[10] = {QQ, DPP, RHO, UU, B1, B2, B3, U1, U2, U3};
   constexpr int ord8[8] = {RHO, UU, B1, B2, B3, U1, U2, U3};
@@ -117,19 +143,20 @@ __host__ __device__ constexpr int fd_order(int s) {
 #endif
 }
 
-template <int J, int N, int BLOCK, class A, class Prob>
+template <int S, int N, bool RED, int BLOCK, class A, class Prob, bool DONE = (S == Unknowns<N, RED>::M)>
 struct FdColumns {
   static __device__ __forceinline__ void run(A &ar, const Prob &prob, const SolverParams &sp, const double (&P)[N],
                                              const Pieces &base, const double (&R0)[N],
-                                             const JacView<N, BLOCK> &jac, bool &singular) {
-    fd_column<fd_order<N>(J), N, BLOCK>(ar, prob, sp, P, base, R0, jac, singular);
-    FdColumns<J + 1, N, BLOCK, A, Prob>::run(ar, prob, sp, P, base, R0, jac, singular);
+                                             const JacView<Unknowns<N, RED>::M, BLOCK> &jac, bool &singular) {
+    fd_column<fd_order<N, RED>(S), N, RED, BLOCK>(ar, prob, sp, P, base, R0, jac, singular);
+    FdColumns<S + 1, N, RED, BLOCK, A, Prob>::run(ar, prob, sp, P, base, R0, jac, singular);
   }
 };
-template <int N, int BLOCK, class A, class Prob>
-struct FdColumns<N, N, BLOCK, A, Prob> {
+template <int S, int N, bool RED, int BLOCK, class A, class Prob>
+struct FdColumns<S, N, RED, BLOCK, A, Prob, true> {
   static __device__ __forceinline__ void run(A &, const Prob &, const SolverParams &, const double (&)[N], const Pieces &,
-                                             const double (&)[N], const JacView<N, BLOCK> &, bool &) {}
+                                             const double (&)[N], const JacView<Unknowns<N, RED>::M, BLOCK> &,
+                                             bool &) {}
 };
 
 // Solves J x = b (b in, x out) for the Jacobian held in shared memory.  Returns false if a pivot is zero or
@@ -214,26 +241,28 @@ __device__ __forceinline__ double linesearch_lambda(A &ar, double f0, double fla
 
 // Runs at most max_iters further Newton iterations (<= 0: until terminal) of one zone.  P, iters, status carry
 // the zone's state between calls.  Returns ||R(P)||_2 of the final state.
-template <int N, int BLOCK, class A, class Prob>
+template <int N, bool RED, int BLOCK, class A, class Prob>
 __device__ __forceinline__ double newton_zone(A &ar, const Prob &prob, const SolverParams &sp, double tol, double (&P)[N],
                                               int &iters, int &status, int max_iters,
-                                              const JacView<N, BLOCK> &jac, int &backtracks) {
+                                              const JacView<Unknowns<N, RED>::M, BLOCK> &jac, int &backtracks) {
+  using U = Unknowns<N, RED>;
+  constexpr int M = U::M;
   double R0[N];
   Pieces pc;
   int k = iters, st = status, done = 0;
   eval_full<N>(ar, prob, P, pc, R0);
-  double f0 = norm2sq<N>(R0);
+  double f0 = norm2sq_rows<N, RED>(R0);
   if (!isfinite(f0)) {
     status = st | ST_NONFINITE;
     return ExactArith().sqrt(f0);
   }
   while (!(ar.sqrt_z(f0) < tol) && k < sp.kmax && (max_iters <= 0 || done < max_iters)) {
     bool singular = false;
-    FdColumns<0, N, BLOCK, A, Prob>::run(ar, prob, sp, P, pc, R0, jac, singular);
-    double dP[N];
+    FdColumns<0, N, RED, BLOCK, A, Prob>::run(ar, prob, sp, P, pc, R0, jac, singular);
+    double dP[M];
 #pragma unroll
-    for (int v = 0; v < N; v++) dP[v] = -R0[v];
-    bool ok = lu_solve<N, BLOCK>(ar, jac, dP);
+    for (int v = 0; v < M; v++) dP[v] = -R0[U::prim(v)];
+    bool ok = lu_solve<M, BLOCK>(ar, jac, dP);
     if (singular || !ok) {
       st |= ST_SINGULAR;
       break;
@@ -243,9 +272,11 @@ __device__ __forceinline__ double newton_zone(A &ar, const Prob &prob, const Sol
     double Pt[N], Rt[N];
     for (int ls = 0; ls <= sp.lsmax; ls++) {
 #pragma unroll
-      for (int v = 0; v < N; v++) Pt[v] = P[v] + lam * dP[v];
+      for (int v = 0; v < N; v++) Pt[v] = P[v];  // the fixed B^i of the reduced solve
+#pragma unroll
+      for (int v = 0; v < M; v++) Pt[U::prim(v)] = P[U::prim(v)] + lam * dP[v];
       eval_full<N>(ar, prob, Pt, pc, Rt);
-      ft = norm2sq<N>(Rt);
+      ft = norm2sq_rows<N, RED>(Rt);
       if (isfinite(ft) && ar.sqrt_z(ft) < ar.sqrt_z(f0) * (1.0 - sp.eps_bt * lam)) {
         accepted = true;
         break;

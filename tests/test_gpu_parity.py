@@ -282,3 +282,35 @@ def test_flux_ct_matches_oracle(n, dim, nvar, recon):
         _, _, Pn, _ = run_steps(dict(gk, flux_ct=False), P0, 1, dt)
         _, _, P1, _ = run_steps(gk, P0, 1, dt)
         assert not np.array_equal(go.interior(Pn)[5:8], go.interior(P1)[5:8])
+
+
+RED_CASES = [((37, 29, 1), 2, 8, og.MINMOD, False), ((33, 21, 1), 2, 10, og.MP5, True),
+             ((19, 13, 11), 3, 10, og.MP5, False), ((19, 13, 11), 3, 8, og.MINMOD, True)]
+
+
+@pytest.mark.parametrize("n,dim,nvar,recon,ct", RED_CASES)
+def test_reduced_solve_matches_oracle(n, dim, nvar, recon, ct):
+    """Reduced solve (L148, L643): B^i explicit, Newton on the other nvar - 3 primitives with a
+    5 x 5 / 7 x 7 Jacobian.  Three time steps bit-identical to the oracle's reduced solve, statistics included."""
+    gk = grid_desc(n, dim, nvar, recon, reduced=True, flux_ct=ct)
+    go, P0 = make_state(gk, 23)
+    dt = go.choose_dt(P0)
+    go, Po, Pc, stats = run_steps(gk, P0, 3, dt)
+    check_stats(stats)
+    assert np.array_equal(go.interior(Pc), go.interior(Po))
+    # iteration by iteration through grim_newton_step as well (P, ||R||, status, iters after every call)
+    gc = cuda_grid(gk)
+    C_, G_, _ = go.stage_prepare(P0, P0, 0.5 * dt)
+    Pit, dPit = P0.copy(), to_dev(P0)
+    state = None
+    drn, dst, dit = gc.zeros(), gc.zeros(dtype=__import__("torch").int32), gc.zeros(dtype=__import__("torch").int32)
+    for call in range(4):
+        nact_o, state, _ = go.newton(P0, P0, C_, G_, 0.5 * dt, Pit, max_iters=1, state=state)
+        nact_c = gc.newton_step(to_dev(P0), to_dev(P0), to_dev(C_), to_dev(G_), 0.5 * dt, 1, dPit, drn, dst, dit)
+        assert nact_c == nact_o
+        assert np.array_equal(go.interior(dPit.cpu().numpy()), go.interior(Pit))
+        assert np.array_equal(go.interior(dst.cpu().numpy()), go.interior(state[1]))
+        assert np.array_equal(go.interior(drn.cpu().numpy()), go.interior(state[0]))
+        if nact_o == 0:
+            break
+    assert nact_o == 0
