@@ -15,7 +15,8 @@
  *   conservation, round trip, LU vs LAPACK, MP5/minmod exactness, Newton
  *   behaviour, geometry identities; flux-CT (og_flux_ct, L327-335): corner-centred
  *   div B at round-off in 2-D / 3-D, conservation, 1-D and uniform reductions
- *   (tests/test_oracle_fluxct.py).
+ *   (tests/test_oracle_fluxct.py); reduced solve (L148, L643): same root as the full
+ *   solve, conservation, explicit induction step (tests/test_oracle_reduced.py).
  * Parity unpinned (no printed number or invariant separates the alternatives;
  * listed in DESIGN.md "Readings"): C-3 beyond 2nd-order agreement, C-4 same-state
  * closure, C-5, C-7, C-8, C-9 in Kerr, C-11, C-15, C-16, and the terms
