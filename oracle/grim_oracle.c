@@ -362,6 +362,12 @@ void og_llf(int n, const double *Fm, const double *Fp, const double *Um, const d
   for (int v = 0; v < n; v++) F[v] = 0.5 * (Fp[v] + Fm[v]) - 0.5 * c * (Up[v] - Um[v]);
 }
 
+/* eq 18 (L170) */
+void og_hlle(int n, const double *Fm, const double *Fp, const double *Um, const double *Up, double cR, double cL,
+             double *F) {
+  for (int v = 0; v < n; v++) F[v] = (cR * Fm[v] + cL * Fp[v] - cR * cL * (Up[v] - Um[v])) / (cL + cR);
+}
+
 /* ===================================================================================
  * O-9 pieces: dense LU with partial pivoting (eq 21; L434 "LAPACK" -> dgesv semantics; C-19),
  * line-search update (eq 25)
@@ -681,13 +687,19 @@ static void face_flux(const og_grid *g, const double *PE, int dir, int i, int j,
   flux_vector(&g->m, gf, tau, 0, Pp, &sp, Up);
   flux_vector(&g->m, gf, tau, dir + 1, Pm, &sm, Fm);
   flux_vector(&g->m, gf, tau, dir + 1, Pp, &sp, Fp);
-  double vp, vm;
+  double vp, vm, vp2, vm2;
   wave_speeds_state(&g->m, gf, tau, dir + 1, Pm, &sm, &vp, &vm);
   double cm = fmax(fabs(vp), fabs(vm));
-  wave_speeds_state(&g->m, gf, tau, dir + 1, Pp, &sp, &vp, &vm);
-  double cp = fmax(fabs(vp), fabs(vm));
+  wave_speeds_state(&g->m, gf, tau, dir + 1, Pp, &sp, &vp2, &vm2);
+  double cp = fmax(fabs(vp2), fabs(vm2));
   double c = fmax(cm, cp);                     /* L164: c_max >= max |c^+-| over both states */
-  og_llf(nv, Fm, Fp, Um, Up, c, F);
+  if (g->d.riemann == OG_HLLE) {               /* L168: bounds on the right- and left-going speeds of both states */
+    double cR = fmax(0.0, fmax(fmax(vp, vm), fmax(vp2, vm2)));
+    double cL = fmax(0.0, fmax(fmax(-vp, -vm), fmax(-vp2, -vm2)));
+    og_hlle(nv, Fm, Fp, Um, Up, cR, cL, F);
+  } else {
+    og_llf(nv, Fm, Fp, Um, Up, c, F);
+  }
   *cface = c;
 }
 

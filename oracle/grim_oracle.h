@@ -37,7 +37,7 @@ enum { OG_RHO = 0, OG_UU = 1, OG_U1 = 2, OG_U2 = 3, OG_U3 = 4,
 
 enum { OG_MINKOWSKI = 0, OG_KERR_MKS = 1 };
 enum { OG_MINMOD = 0, OG_MP5 = 1 };
-enum { OG_LLF = 0 };
+enum { OG_LLF = 0, OG_HLLE = 1 };
 enum { OG_BC_PERIODIC = 0, OG_BC_OUTFLOW = 1, OG_BC_REFLECT_POLAR = 2, OG_BC_NONE = 3 };
 enum { OG_TAU_CONST = 0, OG_TAU_R32 = 1 };
 
@@ -136,6 +136,10 @@ double   og_grid_get_tau(const og_grid *g, int loc, int64_t idx2d);   /* tau_R o
    (NULL for an inactive direction), valid on faces whose index along a is in [ng, ng+n] and whose transverse
    indices are in [ng-1, ng+n]; on return the B^i entries hold the averaged fluxes on the faces of the interior
    zones.  The cell-corner-centred div B of Toth's scheme is then unchanged by the update to round-off. */
+/* HLLE flux (eq 18): cR >= max(c, 0), cL >= max(-c, 0) over the speeds of both states;
+   F = [cR F^- + cL F^+ - cR cL (U^+ - U^-)] / (cL + cR) */
+void     og_hlle(int n, const double *Fm, const double *Fp, const double *Um, const double *Up, double cR, double cL,
+                 double *F);
 void     og_flux_ct(const og_grid *g, double *const Fface[3]);
 /* stage constant C (nvar x Zg) and explicit EMHD gradient terms G (3 x Zg: Xq, Xd, divx) (L438).
    speeds[0..2] = max_z c^d/dX^d, speeds[3] = max_z sum_d c^d/dX^d */

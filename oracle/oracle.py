@@ -17,6 +17,7 @@ import build as _build  # noqa: E402
 NMAX = 10
 MINKOWSKI, KERR_MKS = 0, 1
 MINMOD, MP5 = 0, 1
+LLF, HLLE = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT_POLAR, BC_NONE = 0, 1, 2, 3
 TAU_CONST, TAU_R32 = 0, 1
 ST_CONVERGED, ST_KMAX, ST_LS_EXHAUSTED, ST_SINGULAR, ST_NONFINITE = 1, 2, 4, 8, 16
@@ -94,6 +95,7 @@ def _declare(L):
     L.og_linesearch_lambda.argtypes = [C.c_double] * 3
     L.og_linesearch_lambda.restype = C.c_double
     L.og_llf.argtypes = [C.c_int, _dp, _dp, _dp, _dp, C.c_double, _dp]
+    L.og_hlle.argtypes = [C.c_int, _dp, _dp, _dp, _dp, C.c_double, C.c_double, _dp]
     L.og_grid_create.argtypes = [C.POINTER(GridDesc)]
     L.og_grid_create.restype = C.c_void_p
     L.og_grid_free.argtypes = [C.c_void_p]
@@ -254,6 +256,13 @@ def linesearch_lambda(f0, flam, lam):
     return lib().og_linesearch_lambda(f0, flam, lam)
 
 
+def hlle(Fm, Fp, Um, Up, cR, cL):
+    Fm, Fp, Um, Up = (np.ascontiguousarray(x, dtype=np.float64) for x in (Fm, Fp, Um, Up))
+    F = np.zeros(len(Fm))
+    lib().og_hlle(len(Fm), _d(Fm), _d(Fp), _d(Um), _d(Up), cR, cL, _d(F))
+    return F
+
+
 def llf(Fm, Fp, Um, Up, c):
     Fm, Fp, Um, Up = [np.ascontiguousarray(x, dtype=np.float64) for x in (Fm, Fp, Um, Up)]
     F = np.zeros_like(Fm)
@@ -281,7 +290,7 @@ class Grid:
     def __init__(self, n1, n2=1, n3=1, ng=3, dim=2, xstart=(0, 0, 0), xend=(1, 1, 1),
                  bc=BC_PERIODIC, nvar=10, recon=MINMOD, limiter_theta=1.0, gam=4.0 / 3.0, phi=1.0, psi=1.0,
                  tau_mode=TAU_CONST, tau=1.0, fd_eps=4e-8, eps_bt=1e-4, atol=0.0, rtol=1e-14, kmax=8,
-                 lsmax=5, cfl=0.5, metric=MINKOWSKI, metric_params=(), flux_ct=False, reduced=False):
+                 lsmax=5, cfl=0.5, metric=MINKOWSKI, metric_params=(), flux_ct=False, reduced=False, riemann=0):
         d = GridDesc()
         d.flux_ct = 1 if flux_ct else 0
         d.reduced = 1 if reduced else 0
@@ -290,7 +299,7 @@ class Grid:
             d.xstart[a], d.xend[a] = float(xstart[a]), float(xend[a])
             for s in range(2):
                 d.bc[a][s] = bc if np.isscalar(bc) else bc[a][s]
-        d.nvar, d.recon, d.limiter_theta, d.riemann = nvar, recon, limiter_theta, 0
+        d.nvar, d.recon, d.limiter_theta, d.riemann = nvar, recon, limiter_theta, riemann
         d.gam, d.phi, d.psi, d.tau_mode, d.tau = gam, phi, psi, tau_mode, tau
         d.fd_eps, d.eps_bt, d.atol, d.rtol, d.kmax, d.lsmax, d.cfl = fd_eps, eps_bt, atol, rtol, kmax, lsmax, cfl
         self.desc = d
