@@ -49,7 +49,7 @@ enum { GRIM_MINKOWSKI = 0, GRIM_KERR_MKS = 1 };
 /* reconstruction (L154-160, L115; MP5: C-6) */
 enum { GRIM_MINMOD = 0, GRIM_MP5 = 1 };
 /* Riemann solver (eq 17) */
-enum { GRIM_LLF = 0 };
+enum { GRIM_LLF = 0, GRIM_HLLE = 1 };
 /* boundary conditions per direction and side (C-11) */
 enum { GRIM_BC_PERIODIC = 0, GRIM_BC_OUTFLOW = 1, GRIM_BC_REFLECT_POLAR = 2, GRIM_BC_NONE = 3 };
 /* damping time scale tau_R: constant, or r^{3/2} (C-11) */
@@ -76,7 +76,7 @@ typedef struct {
   int32_t model;            /* GRIM_IDEAL | GRIM_EMHD                                                       */
   int32_t recon;            /* GRIM_MINMOD | GRIM_MP5                                                       */
   double limiter_theta;     /* generalised-minmod theta in [1,2] (L115, L651); also limits EMHD gradients   */
-  int32_t riemann;          /* GRIM_LLF                                                                     */
+  int32_t riemann;          /* GRIM_LLF (eq 17) | GRIM_HLLE (eq 18)                                (L162-172) */
   double gamma;             /* adiabatic index                                                     (L248)   */
   double phi, psi;          /* closure chi = phi cs^2 tau_R, nu = psi cs^2 tau_R                   (L299)   */
   int32_t tau_mode;         /* GRIM_TAU_CONST | GRIM_TAU_R32                                                */

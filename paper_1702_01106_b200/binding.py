@@ -11,7 +11,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 IDEAL, EMHD = 8, 10
 MINKOWSKI, KERR_MKS = 0, 1
 MINMOD, MP5 = 0, 1
-LLF = 0
+LLF, HLLE = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT_POLAR, BC_NONE = 0, 1, 2, 3
 TAU_CONST, TAU_R32 = 0, 1
 ST_CONVERGED, ST_KMAX, ST_LS_EXHAUSTED, ST_SINGULAR, ST_NONFINITE = 1, 2, 4, 8, 16
@@ -127,7 +127,7 @@ class Grid:
     def __init__(self, n1, n2=1, n3=1, ng=3, dim=2, xstart=(0.0, 0.0, 0.0), xend=(1.0, 1.0, 1.0), bc=BC_PERIODIC,
                  model=EMHD, recon=MINMOD, limiter_theta=1.0, gamma=4.0 / 3.0, phi=1.0, psi=1.0, tau_mode=TAU_CONST,
                  tau=1.0, fd_eps=4e-8, eps_bt=1e-4, atol=0.0, rtol=1e-14, kmax=8, lsmax=5, cfl=0.5,
-                 metric=MINKOWSKI, metric_params=(), device=0, stream=None, flux_ct=False, reduced=False):
+                 metric=MINKOWSKI, metric_params=(), device=0, stream=None, flux_ct=False, reduced=False, riemann=LLF):
         import torch
         self.torch = torch
         d = GridDesc()
@@ -136,7 +136,7 @@ class Grid:
             d.xstart[a], d.xend[a] = float(xstart[a]), float(xend[a])
             for s in range(2):
                 d.bc[a][s] = bc if isinstance(bc, int) else bc[a][s]
-        d.model, d.recon, d.limiter_theta, d.riemann = model, recon, limiter_theta, LLF
+        d.model, d.recon, d.limiter_theta, d.riemann = model, recon, limiter_theta, riemann
         d.gamma, d.phi, d.psi, d.tau_mode, d.tau = gamma, phi, psi, tau_mode, tau
         d.fd_eps, d.eps_bt, d.atol, d.rtol, d.kmax, d.lsmax, d.cfl = fd_eps, eps_bt, atol, rtol, kmax, lsmax, cfl
         d.device = device

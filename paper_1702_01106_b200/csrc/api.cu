@@ -155,7 +155,8 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   if (d->dim < 1 || d->dim > 3) return fail(c, GRIM_EINVAL, "dim must be 1, 2 or 3");
   if (d->model != GRIM_IDEAL && d->model != GRIM_EMHD) return fail(c, GRIM_EINVAL, "model must be 8 or 10");
   if (d->recon != GRIM_MINMOD && d->recon != GRIM_MP5) return fail(c, GRIM_EINVAL, "unknown reconstruction");
-  if (d->riemann != GRIM_LLF) return fail(c, GRIM_EINVAL, "only the LLF flux (eq 17) is implemented");
+  if (d->riemann != GRIM_LLF && d->riemann != GRIM_HLLE)
+    return fail(c, GRIM_EINVAL, "riemann must be GRIM_LLF (eq 17) or GRIM_HLLE (eq 18)");
   const int nn[3] = {d->n1, d->n2, d->n3};
   const int need = d->recon == GRIM_MP5 ? 3 : 2;
   if (d->ng < need) return fail(c, GRIM_EINVAL, "ghost depth too small for the reconstruction");
@@ -194,6 +195,7 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   gv.dim = d->dim;
   gv.nvar = d->model;
   gv.recon = d->recon;
+  gv.riemann = d->riemann;
   gv.metric = -1;
   gv.nint = 1;
   gv.zg = 1;

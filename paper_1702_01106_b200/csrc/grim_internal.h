@@ -23,7 +23,7 @@ enum { CONN_NCOMP = 64 };  // Gamma^l_{mn} at [l*16 + m*4 + n]
 
 struct GridView {
   int n[3], ngd[3], sz[3];
-  int dim, nvar, recon, metric;
+  int dim, nvar, recon, metric, riemann;
   long long zg, n2d, nint;   // padded zones, padded 2-D zones, interior zones
   double dx[3], idx[3];
   double xstart[3];

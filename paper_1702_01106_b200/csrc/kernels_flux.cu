@@ -62,13 +62,24 @@ __device__ __forceinline__ void face_compute(A &ar, const GridView &gv, const S 
   flux_vector<N>(g, 0, Pp, sp.th, sp.v, sp.b, sp.h, Up);
   flux_vector<N>(g, DIR + 1, Pm, sm.th, sm.v, sm.b, sm.h, Fm);
   flux_vector<N>(g, DIR + 1, Pp, sp.th, sp.v, sp.b, sp.h, Fp);
-  const double cm =
-      cmax_dir(ar, g, vmax2<N>(ar, gv.m, tau, Pm[RHO], Pm[UU], sm.b.bsq), sm.v.ucon[0], sm.v.ucon[DIR + 1]);
-  const double cp =
-      cmax_dir(ar, g, vmax2<N>(ar, gv.m, tau, Pp[RHO], Pp[UU], sp.b.bsq), sp.v.ucon[0], sp.v.ucon[DIR + 1]);
+  double vpm, vnm, vpp, vnp;  // upper / lower speed bound of the minus state, of the plus state
+  wave_speeds_dir(ar, g, vmax2<N>(ar, gv.m, tau, Pm[RHO], Pm[UU], sm.b.bsq), sm.v.ucon[0], sm.v.ucon[DIR + 1], vpm,
+                  vnm);
+  wave_speeds_dir(ar, g, vmax2<N>(ar, gv.m, tau, Pp[RHO], Pp[UU], sp.b.bsq), sp.v.ucon[0], sp.v.ucon[DIR + 1], vpp,
+                  vnp);
+  const double cm = fmax(fabs(vpm), fabs(vnm));
+  const double cp = fmax(fabs(vpp), fabs(vnp));
   c = fmax(cm, cp);  // L164: c_max >= max |c^+-| over both states
+  if (gv.riemann == 1) {  // HLLE, eq 18 (L168-170): bounds on the right- and left-going speeds of both states
+    const double cR = fmax(0.0, fmax(fmax(vpm, vnm), fmax(vpp, vnp)));
+    const double cL = fmax(0.0, fmax(fmax(-vpm, -vnm), fmax(-vpp, -vnp)));
+    const double den = cL + cR;
 #pragma unroll
-  for (int v = 0; v < N; v++) F[v] = 0.5 * (Fp[v] + Fm[v]) - 0.5 * c * (Up[v] - Um[v]);  // eq 17
+    for (int v = 0; v < N; v++) F[v] = ar.div_z(cR * Fm[v] + cL * Fp[v] - cR * cL * (Up[v] - Um[v]), den);
+  } else {
+#pragma unroll
+    for (int v = 0; v < N; v++) F[v] = 0.5 * (Fp[v] + Fm[v]) - 0.5 * c * (Up[v] - Um[v]);  // eq 17
+  }
 }
 
 template <int N, int RECON, class G, int DIR>

@@ -255,7 +255,8 @@ __device__ __forceinline__ double vmax2(A &ar, const ModelParams &m, double tau,
 // Grid-frame bound along direction d (1..3) of waves moving at +-v_max in the fluid frame (L303; O-4):
 // (k.u)^2 = vmax^2 (g^{mn} + u^m u^n) k_m k_n, k = (-v, delta^d)
 template <class A, class G>
-__device__ __forceinline__ double cmax_dir(A &ar, const G &g, double vm2, double ut, double ud) {
+__device__ __forceinline__ void wave_speeds_dir(A &ar, const G &g, double vm2, double ut, double ud, double &vp,
+                                                double &vn) {
   double g00, g0d, gdd;
   if constexpr (G::flat) {
     g00 = -1.0;
@@ -271,8 +272,13 @@ __device__ __forceinline__ double cmax_dir(A &ar, const G &g, double vm2, double
   double qc = ud * ud - (gdd + ud * ud) * vm2;
   double disc = ar.sqrt_z(fmax(qb * qb - 4.0 * qa * qc, 0.0));
   double i2A = ar.rcp(2.0 * qa);
-  double vp = (qb + disc) * i2A;
-  double vn = (qb - disc) * i2A;
+  vp = (qb + disc) * i2A;
+  vn = (qb - disc) * i2A;
+}
+template <class A, class G>
+__device__ __forceinline__ double cmax_dir(A &ar, const G &g, double vm2, double ut, double ud) {
+  double vp, vn;
+  wave_speeds_dir(ar, g, vm2, ut, ud, vp, vn);
   return fmax(fabs(vp), fabs(vn));
 }
 

@@ -314,3 +314,22 @@ def test_reduced_solve_matches_oracle(n, dim, nvar, recon, ct):
         if nact_o == 0:
             break
     assert nact_o == 0
+
+
+@pytest.mark.parametrize("n,dim,nvar,recon", [((37, 29, 1), 2, 8, og.MINMOD), ((19, 13, 11), 3, 10, og.MP5)])
+def test_hlle_matches_oracle(n, dim, nvar, recon):
+    """HLLE flux (eq 18): stage constants and three time steps bit-identical to the oracle."""
+    gk = grid_desc(n, dim, nvar, recon, riemann=og.HLLE)
+    go, P0 = make_state(gk, 29)
+    gc = cuda_grid(gk)
+    dt = go.choose_dt(P0)
+    C_, G_ = gc.zeros(nvar), gc.zeros(3)
+    gc.compute_fluxes(to_dev(P0), to_dev(P0), 0.5 * dt, C_, G_)
+    Co, _, _ = go.stage_prepare(P0, P0, 0.5 * dt)
+    assert np.array_equal(go.interior(C_.cpu().numpy()), go.interior(Co))
+    go, Po, Pc, stats = run_steps(gk, P0, 3, dt)
+    check_stats(stats)
+    assert np.array_equal(go.interior(Pc), go.interior(Po))
+    _, _, Pl, _ = run_steps(dict(gk, riemann=og.LLF), P0, 1, dt)
+    _, _, Ph, _ = run_steps(gk, P0, 1, dt)
+    assert not np.array_equal(Pl, Ph)
