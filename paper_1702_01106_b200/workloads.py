@@ -125,3 +125,18 @@ def kerr_synthetic(n1=256, n2=256, n3=128, nvar=10, seed=9375, a=0.9375, h=0.3):
     rng = np.random.Generator(np.random.PCG64(seed))
     P *= 1 + 1e-3 * rng.standard_normal(P.shape)
     return grid, P
+
+
+def firehose(n=64, alpha=1e-6):
+    """Firehose-instability test of the paper (L583-601, eqs 58-65): 1-D Minkowski, periodic on [0,1], EMHD,
+    rho = 1, u = 2, B^1 = 0.1, dP = -0.011 < -b^2, tau_R = 1e6, u^2 = 0.1628 alpha sin(2 pi x^1),
+    B^2 = 0.9867 alpha cos(2 pi x^1) (eq 63 prints x^2, a misprint: the mode varies along B^1; reading G-12) --
+    the linearly unstable Alfven mode with growth rate 0.1036.  Returns (grid description, P)."""
+    grid = dict(n1=n, n2=1, n3=1, ng=3, dim=1, xstart=(0.0, 0.0, 0.0), xend=(1.0, 1.0, 1.0), nvar=10, recon=1,
+                limiter_theta=1.0, gam=4.0 / 3.0, phi=1.0, psi=1.0, tau=1e6, rtol=1e-13, kmax=10, lsmax=5, cfl=0.5)
+    X1, _, _ = padded_centres((n, 1, 1), (3, 0, 0), grid["xstart"], grid["xend"])
+    P = np.zeros((10,) + X1.shape)
+    P[0], P[1], P[5], P[9] = 1.0, 2.0, 0.1, -0.011
+    P[3] = 0.1628 * alpha * np.sin(2 * np.pi * X1)
+    P[6] = 0.9867 * alpha * np.cos(2 * np.pi * X1)
+    return grid, P

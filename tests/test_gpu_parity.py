@@ -333,3 +333,17 @@ def test_hlle_matches_oracle(n, dim, nvar, recon):
     _, _, Pl, _ = run_steps(dict(gk, riemann=og.LLF), P0, 1, dt)
     _, _, Ph, _ = run_steps(gk, P0, 1, dt)
     assert not np.array_equal(Pl, Ph)
+
+
+def test_firehose_workload_matches_oracle():
+    """The paper's firehose test (L583-601): background pressure anisotropy dP < -b^2, tau_R = 1e6.
+    Forty steps bit-identical to the oracle, and the unstable mode has grown."""
+    from paper_1702_01106_b200 import workloads
+    gk, P0 = workloads.firehose(n=150, alpha=1e-6)
+    go = oracle_grid(gk)
+    go.fill_ghosts(P0)
+    dt = go.choose_dt(P0)
+    go, Po, Pc, stats = run_steps(gk, P0, 40, dt)
+    check_stats(stats)
+    assert np.array_equal(go.interior(Pc), go.interior(Po))
+    assert abs(go.interior(Pc)[6]).max() > abs(go.interior(P0)[6]).max()
