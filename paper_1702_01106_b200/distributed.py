@@ -30,6 +30,9 @@ def exchange_x3(P, ng, world, rank, periodic=True, group=None):
     hi = rank + 1 if rank < world - 1 else (0 if periodic else None)
     send_lo = P[:, ng:2 * ng].contiguous()             # my lowest interior planes -> lower neighbour's upper ghosts
     send_hi = P[:, n3:n3 + ng].contiguous()            # my highest interior planes -> upper neighbour's lower ghosts
+    if P.is_cuda and dist.get_backend(group) == "gloo":
+        # gloo moves host memory only: stage the planes through the host (the NCCL path is device to device)
+        send_lo, send_hi = send_lo.cpu(), send_hi.cpu()
     recv_lo, recv_hi = torch.empty_like(send_lo), torch.empty_like(send_hi)
     # Message kinds: "up" (tag 0) = my highest interior planes -> upper neighbour's lower ghosts; "down" (tag 1) =
     # my lowest interior planes -> lower neighbour's upper ghosts.  Sends are posted (up, down) and receives
