@@ -3,9 +3,13 @@
 //     C = -U(P_n)/dt' + div F(P_E) - S^E(P_E)                                       (L438; eq 19 / eq 13; C-5)
 // plus, for EMHD, the spatial-gradient terms (Xq, Xd, divx) of the relaxation targets (eqs 37-38; O-8).
 //
-//   face_flux_kernel<DIR> : one thread per lower face of direction DIR; reconstructs the two face states from
-//                           the 4- (minmod) or 6-point (MP5) stencil, evaluates U, F^DIR, c at both with the
-//                           face-centre geometry (C-8) and stores the LLF flux and the face speed.
+//   face_flux_kernel<DIR> : one thread per lower face of direction DIR, on block tiles whose stencil zones are
+//                           staged in shared memory; reconstructs the two face states from the 4- (minmod) or
+//                           6-point (MP5) stencil, evaluates U, F^DIR, c at both with the face-centre geometry
+//                           (C-8) and stores the LLF (eq 17) or HLLE (eq 18) flux and the face speed.
+//   face_box_kernel<DIR>  : the same for the faces the tiles leave out (upper boundary plane; with flux-CT the
+//                           transverse ghost fringe), stencil read directly.
+//   emf_kernel            : flux-CT, face -> edge averages (L327-335).
 //   stage_const_kernel    : one thread per interior zone; differences the face fluxes, adds -U(P_n)/dt' and the
 //                           explicit sources, limited slopes of the derived quantities, max wave-speed figures.
 #include "grim_internal.h"

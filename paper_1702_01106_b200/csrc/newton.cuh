@@ -6,7 +6,8 @@
 //     run-time row index), factorised by a left-looking LU with partial pivoting whose row exchanges are
 //     exchanges of row *pointers* held in registers (eq 21; L434 "LAPACK" -> dgetf2/dgesv semantics: pivot =
 //     first row of maximal |a_ik|, multipliers formed with the reciprocal of the pivot; C-19),
-//   * quadratic backtracking line search (L218-235, eqs 24-25; G-2, C-14).
+//   * quadratic backtracking line search (L218-235, eqs 24-25; G-2, C-14),
+//   * over all N primitives (BASELINE) or, reduced solve, over the N - 3 that have implicit terms (L148, L643).
 // The left-looking order applies to every matrix element the same updates in the same order (k ascending) as
 // the textbook right-looking elimination, so the factors are identical; it reads each multiplier column from
 // shared memory once per later column and writes each element once.
