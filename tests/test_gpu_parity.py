@@ -347,3 +347,14 @@ def test_firehose_workload_matches_oracle():
     check_stats(stats)
     assert np.array_equal(go.interior(Pc), go.interior(Po))
     assert abs(go.interior(Pc)[6]).max() > abs(go.interior(P0)[6]).max()
+
+
+@pytest.mark.parametrize("nvar,ct", [(8, False), (10, True)])
+def test_minmod_with_two_ghost_zones(nvar, ct):
+    """ng = 2 is enough for minmod (G-9): tiles, edge / fringe boxes and the EMHD slopes stay inside the padded array."""
+    gk = grid_desc((41, 23, 1), 2, nvar, og.MINMOD, ng=2, flux_ct=ct)
+    go, P0 = make_state(gk, 5)
+    dt = go.choose_dt(P0)
+    go, Po, Pc, stats = run_steps(gk, P0, 2, dt)
+    check_stats(stats)
+    assert np.array_equal(go.interior(Pc), go.interior(Po))
