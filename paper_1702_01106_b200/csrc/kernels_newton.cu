@@ -38,6 +38,7 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
     load_geom<0>(gv.geomC, gv.n2d, (long long)j * gv.sz[0] + i, prob.g, prob.tau_);
   }
   double P[N];
+  Pieces pc0;
   {
     double Pn_z[N], PE_z[N];
 #pragma unroll
@@ -62,13 +63,14 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
       prob.Xd = a.Gx[1 * gv.zg + z];
       prob.divx = a.Gx[2 * gv.zg + z];
     }
-    prob.setup(ar, Pn_z, PE_z, a.dt_stage);
+    full_state<N>(ar, prob.m, prob.g, prob.tau_, P, pc0.th, pc0.v, pc0.b, pc0.h);
+    prob.setup(ar, Pn_z, PE_z, a.dt_stage, pc0, !RED && a.PE == a.Pguess, !RED && a.Pn == a.Pguess);
   }
   const double tol = gv.sp.atol + gv.sp.rtol * prob.scale;
   int it = a.fresh ? 0 : a.iters[z];
   int nbt = 0;
   JacView<M, NB> jac{sj};
-  double rn = newton_zone<N, RED, NB>(ar, prob, gv.sp, tol, P, it, st, a.max_iters, jac, nbt);
+  double rn = newton_zone<N, RED, NB>(ar, prob, gv.sp, tol, P, it, st, a.max_iters, jac, nbt, &pc0);
   if (!ar.good()) return -1;
 #pragma unroll
   for (int v = 0; v < N; v++) a.Piter[v * gv.zg + z] = P[v];

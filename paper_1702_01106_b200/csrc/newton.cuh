@@ -245,13 +245,19 @@ __device__ __forceinline__ double linesearch_lambda(A &ar, double f0, double fla
 template <int N, bool RED, int BLOCK, class A, class Prob>
 __device__ __forceinline__ double newton_zone(A &ar, const Prob &prob, const SolverParams &sp, double tol, double (&P)[N],
                                               int &iters, int &status, int max_iters,
-                                              const JacView<Unknowns<N, RED>::M, BLOCK> &jac, int &backtracks) {
+                                              const JacView<Unknowns<N, RED>::M, BLOCK> &jac, int &backtracks,
+                                              const Pieces *pc0 = nullptr) {
   using U = Unknowns<N, RED>;
   constexpr int M = U::M;
   double R0[N];
   Pieces pc;
   int k = iters, st = status, done = 0;
-  eval_full<N>(ar, prob, P, pc, R0);
+  if (pc0) {  // the caller has the state pieces of P already
+    pc = *pc0;
+    prob.assemble(P, pc, R0);
+  } else {
+    eval_full<N>(ar, prob, P, pc, R0);
+  }
   double f0 = norm2sq_rows<N, RED>(R0);
   if (!isfinite(f0)) {
     status = st | ST_NONFINITE;

@@ -28,11 +28,16 @@ struct StageProblem {
 
   // Everything that depends only on P_n and P_E (L438)
   template <class A>
-  __device__ __forceinline__ void setup(A &ar, const double (&Pn)[N], const double (&PE)[N], double dt_stage) {
+  // pc0: the state pieces of the initial iterate, already computed by the caller.  In grim_timestep the guess is
+  // P_E, and in its first stage P_n is P_E too: the states of P_E / P_n are then pc0 itself (same inputs, same code,
+  // same bits) and are not computed again.
+  __device__ __forceinline__ void setup(A &ar, const double (&Pn)[N], const double (&PE)[N], double dt_stage,
+                                        const Pieces &pc0, bool pe_is_guess, bool pn_is_guess) {
     idt = ar.rcp(dt_stage);
     itau = ar.rcp(tau_);
     Pieces pn;
-    full_state<N>(ar, m, g, tau_, Pn, pn.th, pn.v, pn.b, pn.h);
+    if (pn_is_guess) pn = pc0;
+    else full_state<N>(ar, m, g, tau_, Pn, pn.th, pn.v, pn.b, pn.h);
     double Un[N];
     flux_vector<N>(g, 0, Pn, pn.th, pn.v, pn.b, pn.h, Un);
     scale = ar.sqrt_z(norm2sq<N>(Un)) * idt;
@@ -44,7 +49,8 @@ struct StageProblem {
       qtn = Pn[QQ] * pn.th.fq;
       dtn = Pn[DPP] * pn.th.fdp;
       Pieces pe;
-      full_state<N>(ar, m, g, tau_, PE, pe.th, pe.v, pe.b, pe.h);
+      if (pe_is_guess) pe = pc0;
+      else full_state<N>(ar, m, g, tau_, PE, pe.th, pe.v, pe.b, pe.h);
 #pragma unroll
       for (int i = 0; i < 4; i++) bh[i] = pe.h.con[i];
       ThE = pe.th.Th;
