@@ -272,6 +272,7 @@ struct TileFlux {
 // Stage constant, EMHD gradient terms and wave-speed figures of padded zone z under arithmetic policy A
 template <int N, class G, bool CT, class A, class FS>
 __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, const FS &fs,
+                                                    const double (&Pn_z)[N], const double (&PE_z)[N],
                                                     const double *__restrict__ PE,
                                                     const double *__restrict__ Pn, double dt_stage,
                                                     const double *__restrict__ Fface,
@@ -283,12 +284,6 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
   double tau = gv.tau_const;
   if constexpr (!G::flat) load_geom<0>(gv.geomC, gv.n2d, id, gc, tau);
 
-  double Pn_z[N], PE_z[N];
-#pragma unroll
-  for (int v = 0; v < N; v++) {
-    Pn_z[v] = Pn[v * gv.zg + z];
-    PE_z[v] = PE[v * gv.zg + z];
-  }
   Pieces sn, sE;
   full_state<N>(ar, gv.m, gc, tau, Pn_z, sn.th, sn.v, sn.b, sn.h);
   full_state<N>(ar, gv.m, gc, tau, PE_z, sE.th, sE.v, sE.b, sE.h);
@@ -474,7 +469,12 @@ __device__ __noinline__ void stage_const_replay(const GridView &gv, const double
   ExactArith ar;
   double C_[N], G_[3] = {0.0, 0.0, 0.0}, s_[4] = {0.0, 0.0, 0.0, 0.0};
   const GlobalFlux<N> fs{Fface, gv.zg, z, {1, (long long)gv.sz[0], (long long)gv.sz[0] * gv.sz[1]}};
-  stage_const_compute<N, G, CT>(ar, gv, fs, PE, Pn, dt_stage, Fface, cface, want_speeds, z, id, C_, G_, s_);
+  double Pn_z[N], PE_z[N];
+  for (int v = 0; v < N; v++) {
+    Pn_z[v] = Pn[v * gv.zg + z];
+    PE_z[v] = PE[v * gv.zg + z];
+  }
+  stage_const_compute<N, G, CT>(ar, gv, fs, Pn_z, PE_z, PE, Pn, dt_stage, Fface, cface, want_speeds, z, id, C_, G_, s_);
   for (int v = 0; v < N; v++) Cout[v] = C_[v];
   for (int v = 0; v < 3; v++) Gout[v] = G_[v];
   for (int v = 0; v < 4; v++) sp_loc[v] = s_[v];
@@ -502,7 +502,14 @@ stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict
     double Cout[N], Gout[3] = {0.0, 0.0, 0.0};
     SpecArith ar;
     const GlobalFlux<N> fs{Fface, gv.zg, z, {1, (long long)gv.sz[0], (long long)gv.sz[0] * gv.sz[1]}};
-    stage_const_compute<N, G, CT>(ar, gv, fs, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
+    double Pn_z[N], PE_z[N];
+#pragma unroll
+    for (int v = 0; v < N; v++) {
+      Pn_z[v] = Pn[v * gv.zg + z];
+      PE_z[v] = PE[v * gv.zg + z];
+    }
+    stage_const_compute<N, G, CT>(ar, gv, fs, Pn_z, PE_z, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout,
+                                  Gout, sp_loc);
     if (!ar.good())
       stage_const_replay<N, G, CT>(gv, PE, Pn, dt_stage, Fface, cface, cnt != nullptr, z, id, Cout, Gout, sp_loc);
 #pragma unroll
@@ -539,6 +546,17 @@ stage_const_tiled_kernel(const __grid_constant__ GridView gv, const double *__re
   const int i0 = gv.ngd[0] + (int)blockIdx.x * T0, j0 = gv.ngd[1] + (int)blockIdx.y * T1,
             k = gv.ngd[2] + (int)blockIdx.z;
   const long long zg = gv.zg;
+  // the zone's own primitives are requested first, so that they arrive while the tile is being staged
+  const int t0 = (int)threadIdx.x % T0, t1 = (int)threadIdx.x / T0;
+  const int i = i0 + t0, j = j0 + t1;
+  const bool valid = i < gv.ngd[0] + gv.n[0] && j < gv.ngd[1] + gv.n[1];
+  const long long z = zone_index(gv, valid ? i : gv.ngd[0], valid ? j : gv.ngd[1], k);
+  double Pn_z[N], PE_z[N];
+#pragma unroll
+  for (int v = 0; v < N; v++) {
+    Pn_z[v] = Pn[v * zg + z];
+    PE_z[v] = PE[v * zg + z];
+  }
   // direction 0: faces (i0 .. i0+T0, j0 .. j0+T1-1); direction 1: (i0 .. i0+T0-1, j0 .. j0+T1);
   // direction 2: (i0 .. , j0 .. ) at k and k+1.  Coordinates beyond the padded array are skipped (their zones are not
   // computed either).
@@ -570,15 +588,13 @@ stage_const_tiled_kernel(const __grid_constant__ GridView gv, const double *__re
     }
   }
   __syncthreads();
-  const int t0 = (int)threadIdx.x % T0, t1 = (int)threadIdx.x / T0;
-  const int i = i0 + t0, j = j0 + t1;
-  if (i >= gv.ngd[0] + gv.n[0] || j >= gv.ngd[1] + gv.n[1]) return;
-  const long long z = zone_index(gv, i, j, k);
+  if (!valid) return;
   const long long id = (long long)j * gv.sz[0] + i;
   double Cout[N], Gout[3] = {0.0, 0.0, 0.0}, sp_loc[4];
   SpecArith ar;
   const TF fs{tile, t0, t1};
-  stage_const_compute<N, G, CT>(ar, gv, fs, PE, Pn, dt_stage, Fface, cface, false, z, id, Cout, Gout, sp_loc);
+  stage_const_compute<N, G, CT>(ar, gv, fs, Pn_z, PE_z, PE, Pn, dt_stage, Fface, cface, false, z, id, Cout, Gout,
+                                sp_loc);
   if (!ar.good()) stage_const_replay<N, G, CT>(gv, PE, Pn, dt_stage, Fface, cface, false, z, id, Cout, Gout, sp_loc);
 #pragma unroll
   for (int v = 0; v < N; v++) C[v * zg + z] = Cout[v];
