@@ -285,8 +285,9 @@ __device__ __forceinline__ void stage_const_compute(A &ar, const GridView &gv, c
   if constexpr (!G::flat) load_geom<0>(gv.geomC, gv.n2d, id, gc, tau);
 
   Pieces sn, sE;
-  full_state<N>(ar, gv.m, gc, tau, Pn_z, sn.th, sn.v, sn.b, sn.h);
   full_state<N>(ar, gv.m, gc, tau, PE_z, sE.th, sE.v, sE.b, sE.h);
+  if (G::flat && Pn == PE) sn = sE;  // first stage: P_n is P_E, same state, same bits (general metric: slower)
+  else full_state<N>(ar, gv.m, gc, tau, Pn_z, sn.th, sn.v, sn.b, sn.h);
   double Un[N];
   flux_vector<N>(gc, 0, Pn_z, sn.th, sn.v, sn.b, sn.h, Un);
 
