@@ -87,11 +87,14 @@ __device__ __noinline__ int stage_zone_replay(const GridView &gv, const StageArg
   return stage_zone<N, G, RED>(ar, gv, a, z, i, j, st, sj);
 }
 
+#ifndef GRIM_N8_MINB
+#define GRIM_N8_MINB 2  // ideal MHD: 64 + 8 doubles of shared memory per zone would allow 3 blocks (170 registers)
+#endif
 #ifndef GRIM_RED_MINB
 #define GRIM_RED_MINB 2  // reduced solve: (N-3)^2 + N doubles of shared memory per zone leave room for 3 blocks
 #endif
 template <int N, class G, bool RED>
-__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : 256 / NB)
+__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB))
 newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
@@ -199,7 +202,7 @@ __device__ __noinline__ int invert_zone_replay(const GridView &gv, const InvertA
 }
 
 template <int N>
-__global__ void __launch_bounds__(NB, 256 / NB)
+__global__ void __launch_bounds__(NB, N == 8 ? GRIM_N8_MINB : 256 / NB)
 invert_kernel(const __grid_constant__ GridView gv, const __grid_constant__ InvertArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
