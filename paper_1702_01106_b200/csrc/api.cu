@@ -13,6 +13,14 @@
 
 using namespace grim;
 
+// grim_invert_primitives: Newton iterations per sweep over the compacted active set (first sweep, later sweeps)
+#ifndef GRIM_SWEEP_FIRST
+#define GRIM_SWEEP_FIRST 4
+#endif
+#ifndef GRIM_SWEEP_REST
+#define GRIM_SWEEP_REST 4
+#endif
+
 struct KernelSpan {
   int kclass, launches;
   cudaEvent_t e0, e1;
@@ -411,7 +419,7 @@ extern "C" int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_t
   long long nlist = nz;
   int first = 1, cur = 0, done_iters = 0;
   while (nlist > 0) {
-    const int sweep = first ? 4 : 2;
+    const int sweep = first ? GRIM_SWEEP_FIRST : GRIM_SWEEP_REST;
     CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
     c->launches += timed(c, GRIM_K_INVERT, [&] { return launch_invert(c->gv, nz, nlist, c->list[cur], U_target, P_inout, iters, status, resnorm, sweep,
                                  first, c->list[cur ^ 1], c->cnt, c->stream); });
