@@ -148,6 +148,27 @@ def test_kerr_timestep_bitwise_with_oracle_tables(nvar, recon):
     assert np.array_equal(go.interior(dP.cpu().numpy()), go.interior(Po))
 
 
+@pytest.mark.parametrize("opts", [dict(flux_ct=True), dict(reduced=True), dict(riemann=1),
+                                  dict(flux_ct=True, reduced=True, riemann=1, nvar=8, recon=0)])
+def test_kerr_options_bitwise_with_oracle_tables(opts):
+    """Flux-CT, the reduced solve (B^i_new = -(C_B dt')/sqrt(-g): the division by sqrt(-g) only exists here) and the
+    HLLE flux (general-metric speed bounds) in curved space, oracle tables uploaded: bit-identical time steps."""
+    gk = dict(KERR, **opts)
+    go, gc = oracle_grid(gk), cuda_grid(gk)
+    gc.set_metric_tables(*go.geometry_tables())
+    P0 = kerr_state(go, 6)
+    dt = go.choose_dt(P0)
+    Po, dP = P0.copy(), to_dev(P0)
+    for _ in range(2):
+        so = go.timestep(Po, dt)
+        _, sc = gc.timestep(dP, dt, want_stats=True)
+        for s in range(2):
+            assert list(so.iters_hist[s]) == list(sc.iters_hist[s])
+            assert so.unconverged[s] == sc.unconverged[s]
+    assert np.array_equal(go.interior(dP.cpu().numpy()), go.interior(Po), equal_nan=True)
+    assert np.isfinite(go.interior(Po)).all()
+
+
 @pytest.mark.parametrize("nvar,recon", [(10, og.MP5), (8, og.MINMOD)])
 def test_kerr_timestep_fixed_count_matches_oracle(nvar, recon):
     """The same steps with the library's own geometry precompute (a0).  The geometry tables of the two sides
