@@ -358,3 +358,17 @@ def test_minmod_with_two_ghost_zones(nvar, ct):
     go, Po, Pc, stats = run_steps(gk, P0, 2, dt)
     check_stats(stats)
     assert np.array_equal(go.interior(Pc), go.interior(Po))
+
+
+def test_config3_hundred_steps():
+    """North star: max relative error per primitive <= 1e-8 after 100 steps, identical iteration counts.  Config 3's
+    generator at 16^3, 100 steps: the result is bit-identical."""
+    from paper_1702_01106_b200 import workloads
+    gk, P0 = workloads.config3(n=16)
+    go = oracle_grid(gk)
+    dt = go.choose_dt(P0)
+    go, Po, Pc, stats = run_steps(gk, P0, 100, dt)
+    err = rel_err_per_primitive(Pc, Po, go.interior)
+    assert err.max() <= 1e-8, err
+    check_stats(stats)
+    assert np.array_equal(go.interior(Pc), go.interior(Po))
