@@ -760,6 +760,40 @@ void og_flux_ct(const og_grid *g, double *const Fface[3]) {
   for (int c = 0; c < 3; c++) free(E[c]);
 }
 
+/* Geometric source of the energy-momentum equations (eq 31): S_nu = sqrt(-g) T^kappa_lambda Gamma^lambda_{nu kappa},
+ * nu = 0..3, conn[l][m][n] = Gamma^l_{mn}.  (For the Levi-Civita connection this equals
+ * (1/2) sqrt(-g) T^{kappa lambda} d_nu g_{kappa lambda}, which is what tests/test_oracle_curved.py pins it with.) */
+static void geometric_source(const og_model *m, const og_geom *gc, const double conn[4][4][4], const double *P,
+                             const og_state *s, double S[4]) {
+  double T[4][4];
+  for (int mu = 0; mu < 4; mu++) stress_row(m, P, s, mu, T[mu]);
+  for (int nu = 0; nu < 4; nu++) {
+    double acc = 0.0;
+    for (int kk = 0; kk < 4; kk++)
+      for (int l = 0; l < 4; l++) acc += T[kk][l] * conn[l][nu][kk];
+    S[nu] = gc->sqrtmg * acc;
+  }
+}
+
+/* the same at a point: P padded to OG_NMAX entries is not required (nvar of the model are read) */
+void og_geometric_source(const og_model *m, const og_geom *g, const double conn[4][4][4], const double *P,
+                         double S[4]) {
+  double Pf[OG_NMAX];
+  pad_prims(m, P, Pf);
+  og_state s;
+  get_state(Pf, g, &s);
+  geometric_source(m, g, conn, Pf, &s, S);
+}
+
+/* T^mu_nu of state P (eq 27 lowered; eqs 33-34), row-major T[mu][nu] */
+void og_stress_tensor(const og_model *m, const og_geom *g, const double *P, double T[4][4]) {
+  double Pf[OG_NMAX];
+  pad_prims(m, P, Pf);
+  og_state s;
+  get_state(Pf, g, &s);
+  for (int mu = 0; mu < 4; mu++) stress_row(m, Pf, &s, mu, T[mu]);
+}
+
 /* ===================================================================================
  * O-8  Stage precompute: C = -U(P_n)/dt' + divF(P_E) - S^E(P_E) and the spatial-gradient terms of
  * the EMHD sources (L438, eq 19, eq 13; C-5)
@@ -829,16 +863,7 @@ void og_stage_prepare(const og_grid *g, const double *Pn, const double *PE, doub
           if (ssum > lmax[3]) lmax[3] = ssum;
           /* explicit geometric source sqrt(-g) T^k_l Gamma^l_{nu k} at P_E (eq 31; C-5) */
           double SE[OG_NMAX] = {0};
-          if (g->metric != OG_MINKOWSKI) {
-            double T[4][4];
-            for (int mu = 0; mu < 4; mu++) stress_row(&g->m, PE_z, &sE, mu, T[mu]);
-            for (int nu = 0; nu < 4; nu++) {
-              double s = 0.0;
-              for (int kk = 0; kk < 4; kk++)
-                for (int l = 0; l < 4; l++) s += T[kk][l] * g->conn[id][l][nu][kk];
-              SE[1 + nu] = gc->sqrtmg * s;
-            }
-          }
+          if (g->metric != OG_MINKOWSKI) geometric_source(&g->m, gc, g->conn[id], PE_z, &sE, SE + 1);
           for (int v = 0; v < nv; v++) C[(int64_t)v * zg + z] = -Un[v] * idt + divF[v] - SE[v];
           /* spatial-gradient parts of the EMHD sources: limited 3-point slopes of derived quantities (L115) */
           if (nv == 10) {

@@ -17,10 +17,15 @@
  *   div B at round-off in 2-D / 3-D, conservation, 1-D and uniform reductions
  *   (tests/test_oracle_fluxct.py); reduced solve (L148, L643): same root as the full
  *   solve, conservation, explicit induction step (tests/test_oracle_reduced.py).
+ *   Curved space (tests/test_oracle_curved.py): og_geometric_source against (1/2) T^{kl} d_nu g_kl; the connection
+ *   terms of the EMHD targets against brute-force covariant derivatives; og_stage_prepare + og_zone_residual on Kerr
+ *   grids (2-D and 3-D, all rows, face-centre geometry, tau_R = r^{3/2}, the terms (1/2) q~ div u, (1/2) dP~ div u)
+ *   by a manufactured solution converging at second order to the continuum equations; an exact static Tolman
+ *   atmosphere with a monopole field in Schwarzschild staying stationary at second order; polar reflection against the
+ *   analytic field at the mirrored coordinates.
  * Parity unpinned (no printed number or invariant separates the alternatives;
  * listed in DESIGN.md "Readings"): C-3 beyond 2nd-order agreement, C-4 same-state
- * closure, C-5, C-7, C-8, C-9 in Kerr, C-11, C-15, C-16, and the terms
- * (1/2) q~ div u, (1/2) dP~ div u which vanish at linear order.
+ * closure, C-7, C-9 inside the ergosphere, C-11 (choice of boundary conditions and floors), C-15, C-16.
  */
 #ifndef GRIM_ORACLE_H
 #define GRIM_ORACLE_H
@@ -113,6 +118,11 @@ void   og_emhd_targets(const og_model *m, const og_geom *g, const double conn[4]
                        const double *PE, const double dTheta[4], const double ducov[4][4],
                        double divu, double *q0, double *dP0);
 void   og_rescale_factors(const og_model *m, double tau, const double *P, double *fq, double *fdp);
+/* geometric source S_nu = sqrt(-g) T^kappa_lambda Gamma^lambda_{nu kappa}, nu = 0..3 (eq 31), the routine
+   og_stage_prepare calls per zone; and T^mu_nu itself (eq 27 lowered, eqs 33-34) */
+void   og_geometric_source(const og_model *m, const og_geom *g, const double conn[4][4][4], const double *P,
+                           double S[4]);
+void   og_stress_tensor(const og_model *m, const og_geom *g, const double *P, double T[4][4]);
 double og_minmod3(double a, double b, double c);
 double og_slope(double theta, double vm, double v0, double vp);
 void   og_reconstruct(int recon, double theta, const double v[5], double *left_of_upper, double *right_of_lower);

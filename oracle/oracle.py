@@ -83,6 +83,8 @@ def _declare(L):
     L.og_emhd_targets.argtypes = [C.POINTER(Model), C.POINTER(Geom), _dp, C.c_double, _dp, _dp, _dp,
                                   C.c_double, _dp, _dp]
     L.og_rescale_factors.argtypes = [C.POINTER(Model), C.c_double, _dp, _dp, _dp]
+    L.og_geometric_source.argtypes = [C.POINTER(Model), C.POINTER(Geom), _dp, _dp, _dp]
+    L.og_stress_tensor.argtypes = [C.POINTER(Model), C.POINTER(Geom), _dp, _dp]
     L.og_minmod3.argtypes = [C.c_double] * 3
     L.og_minmod3.restype = C.c_double
     L.og_slope.argtypes = [C.c_double] * 4
@@ -214,6 +216,23 @@ def emhd_targets(m, g, conn, tau, PE, dTheta, ducov, divu):
     lib().og_emhd_targets(C.byref(m), C.byref(g), _d(conn), tau, _d(PE), _d(dTheta), _d(ducov), divu,
                           C.byref(q0), C.byref(dP0))
     return q0.value, dP0.value
+
+
+def geometric_source(m, g, conn, P):
+    """S_nu = sqrt(-g) T^k_l Gamma^l_{nu k}, nu = 0..3 (eq 31), as og_stage_prepare forms it."""
+    P = np.ascontiguousarray(P, dtype=np.float64)
+    conn = np.ascontiguousarray(conn, dtype=np.float64)
+    S = np.zeros(4)
+    lib().og_geometric_source(C.byref(m), C.byref(g), _d(conn), _d(P), _d(S))
+    return S
+
+
+def stress_tensor(m, g, P):
+    """T^mu_nu [mu][nu] of state P."""
+    P = np.ascontiguousarray(P, dtype=np.float64)
+    T = np.zeros((4, 4))
+    lib().og_stress_tensor(C.byref(m), C.byref(g), _d(P), _d(T))
+    return T
 
 
 def rescale_factors(m, tau, P):

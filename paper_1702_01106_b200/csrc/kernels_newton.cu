@@ -125,11 +125,8 @@ static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE
                           int32_t *iters, Counters *cnt, cudaStream_t s) {
   constexpr int M = Unknowns<N, RED>::M;
   const size_t smem = (size_t)(M * M + N) * NB * sizeof(double);  // Jacobian + C per thread
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(newton_stage_kernel<N, G, RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
+  // per device and context, so set before every launch (cheap); a failure surfaces as the launch error
+  cudaFuncSetAttribute(newton_stage_kernel<N, G, RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   const long long blocks = (gv.nint + NB - 1) / NB;
   const StageArgs a{Pn, PE, C, Gx, Pguess, dt_stage, max_iters, fresh, Piter, resnorm, status, iters};
   newton_stage_kernel<N, G, RED><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
@@ -231,11 +228,7 @@ static int launch_invert_t(const GridView &gv, long long nz, long long nlist, co
                            const double *Ustar, double *P, int32_t *iters, int32_t *status, double *resnorm,
                            int max_iters, int first, long long *next_list, Counters *cnt, cudaStream_t s) {
   const size_t smem = (size_t)(N * N + N) * NB * sizeof(double);  // Jacobian + C (or U*) per thread
-  static bool attr_set = false;
-  if (!attr_set) {
-    cudaFuncSetAttribute(invert_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    attr_set = true;
-  }
+  cudaFuncSetAttribute(invert_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   const long long blocks = (nlist + NB - 1) / NB;
   if (blocks == 0) return 0;
   const InvertArgs a{nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list};

@@ -234,6 +234,184 @@ __device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, do
   return ok;
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// The same factorisation by register panels.  Shared memory moves 128 B per cycle and SM -- a warp's 8-byte
+// load costs as much as four of its fp64 instructions -- and the column-at-a-time LU above loads every
+// multiplier once per later column (285 loads for N = 10): the solve was bound by the shared-memory pipe
+// (profiles/r2a_newton_lu_panels.md).  Here a panel of columns is held in registers at a time: the multipliers
+// of the earlier pivots are loaded once per panel, those of the panel's own pivots are never loaded, and the
+// last panel carries the right-hand side along and is never stored -- the back substitution reads its U from
+// the registers.  N = 10 with panels of 5 + 5 columns loads 35 multipliers; N <= 8 is one panel (no stores).
+//
+// Every matrix element still receives the updates of the pivots k = 0, 1, ... in ascending order, each as
+// x - l * x_k with the multiplier l = x * (1/pivot): the same rounded operations as og_lu_solve / dgetf2, so
+// the factors, the pivot sequence (first position of maximal |x_i|) and the solution are identical.  A row
+// exchange swaps two entries of rowoff (for the columns in shared memory) and positions j and p of the panel
+// columns still in registers (select chains; p is a run-time index).
+// ---------------------------------------------------------------------------------------------------------
+template <int M>
+__device__ __forceinline__ void swap_positions(double (&x)[M], int j, int p) {
+  // branch-free: selects on the run-time index p (a conditional assignment would send the column to local memory)
+  const double xj = x[j];
+  double xp = xj;
+#pragma unroll
+  for (int i = j + 1; i < M; i++) xp = (p == i) ? x[i] : xp;
+#pragma unroll
+  for (int i = j + 1; i < M; i++) x[i] = (p == i) ? xj : x[i];
+  x[j] = xp;
+}
+
+// Factorises columns C0 .. C0+CB-1 held in X (pivoted order, updates of the pivots < C0 applied).  RHS: b is
+// carried along as a passenger column.  STORE: the finished columns go to shared memory (L below the
+// diagonal, U above, 1/pivot on it).
+template <int M, int BLOCK, int C0, int CB, bool RHS, bool STORE, class A>
+__device__ __forceinline__ void lu_panel(A &ar, const JacView<M, BLOCK> &jac, int (&rowoff)[M], double (&X)[CB][M],
+                                         double (&b)[M], double (&rinv)[CB], bool &ok) {
+#pragma unroll
+  for (int jj = 0; jj < CB; jj++) {
+    const int j = C0 + jj;
+    // pivot: first position of maximal |x_i|, i >= j
+    int p = j;
+    double xp = X[jj][j], amax = fabs(X[jj][j]);
+#pragma unroll
+    for (int i = j + 1; i < M; i++) {
+      const double v = fabs(X[jj][i]);
+      const bool gt = v > amax;
+      amax = gt ? v : amax;
+      xp = gt ? X[jj][i] : xp;
+      p = gt ? i : p;
+    }
+    ok = ok && (amax > 0.0) && isfinite(amax);
+    const double r = ar.rcp(xp);
+    rinv[jj] = r;
+    // exchange positions j and p
+    const int roj = rowoff[j];
+    int rop = roj;
+#pragma unroll
+    for (int i = j + 1; i < M; i++) rop = (p == i) ? rowoff[i] : rop;
+#pragma unroll
+    for (int i = j + 1; i < M; i++) rowoff[i] = (p == i) ? roj : rowoff[i];
+    rowoff[j] = rop;
+#pragma unroll
+    for (int c = jj; c < CB; c++) swap_positions<M>(X[c], j, p);
+    if (RHS) swap_positions<M>(b, j, p);
+    // multipliers, then the update of the later panel columns and of the right-hand side
+#pragma unroll
+    for (int i = j + 1; i < M; i++) X[jj][i] = X[jj][i] * r;
+#pragma unroll
+    for (int c = jj + 1; c < CB; c++)
+#pragma unroll
+      for (int i = j + 1; i < M; i++) X[c][i] = X[c][i] - X[jj][i] * X[c][j];
+    if (RHS) {
+#pragma unroll
+      for (int i = j + 1; i < M; i++) b[i] = b[i] - X[jj][i] * b[j];
+    }
+    if (STORE) {
+#pragma unroll
+      for (int i = 0; i < M; i++) jac.at(rowoff[i], j) = (i == j) ? r : X[jj][i];
+    }
+  }
+}
+
+// Panel split of the M x M solve.  N = 10: cuts from GRIM_LU_CUTS; smaller systems (ideal MHD, reduced solves,
+// 8 x 8 and below) are one panel, i.e. factorised entirely in registers.
+// GRIM_LU_CUTS: the decimal digits are the interior cuts, ascending (4 -> panels [0,4) [4,10); 2468 -> pairs).
+#ifndef GRIM_LU_CUTS
+#define GRIM_LU_CUTS 4
+#endif
+template <int M>
+struct LuSplit {
+  static constexpr int n = 1;
+  static __host__ __device__ constexpr int b(int) { return 0; }
+  static __host__ __device__ constexpr int e(int) { return M; }
+};
+__host__ __device__ constexpr int lu_cut_count() {
+  int c = 0;
+  for (long long v = GRIM_LU_CUTS; v > 0; v /= 10) c++;
+  return c;
+}
+// boundary q (0 .. count + 1): 0, the digits, 10
+__host__ __device__ constexpr int lu_cut(int q) {
+  if (q <= 0) return 0;
+  if (q > lu_cut_count()) return 10;
+  long long v = GRIM_LU_CUTS;
+  for (int s = 0; s < lu_cut_count() - q; s++) v /= 10;
+  return (int)(v % 10);
+}
+template <>
+struct LuSplit<10> {
+  static constexpr int n = lu_cut_count() + 1;
+  static __host__ __device__ constexpr int b(int pi) { return lu_cut(pi); }
+  static __host__ __device__ constexpr int e(int pi) { return lu_cut(pi + 1); }
+};
+
+// Panel PI and all later ones; the last panel carries b along, is not stored, and ends with the back substitution.
+template <int M, int BLOCK, int PI, class A>
+__device__ __forceinline__ void lu_panels_from(A &ar, const JacView<M, BLOCK> &jac, int (&rowoff)[M], double (&b)[M],
+                                               bool &ok) {
+  using S = LuSplit<M>;
+  constexpr int C0 = S::b(PI), C1 = S::e(PI), CB = C1 - C0;
+  constexpr bool LAST = (PI == S::n - 1);
+  double X[CB][M], rinv[CB];
+  // the panel's columns in pivoted order (the identity for the first panel)
+#pragma unroll
+  for (int c = 0; c < CB; c++)
+#pragma unroll
+    for (int i = 0; i < M; i++)
+      X[c][i] = (C0 == 0) ? jac.at(JacView<M, BLOCK>::row(i), C0 + c) : jac.at(rowoff[i], C0 + c);
+  if (LAST && C0 > 0) {
+    // b into pivoted order through the storage of the last column, which the loads have just emptied
+#pragma unroll
+    for (int i = 0; i < M; i++) jac.at(JacView<M, BLOCK>::row(i), M - 1) = b[i];
+#pragma unroll
+    for (int i = 0; i < M; i++) b[i] = jac.at(rowoff[i], M - 1);
+  }
+  // updates of the earlier panels' pivots, k ascending
+#pragma unroll
+  for (int k = 0; k < C0; k++) {
+#pragma unroll
+    for (int i = k + 1; i < M; i++) {
+      const double l = jac.at(rowoff[i], k);
+#pragma unroll
+      for (int c = 0; c < CB; c++) X[c][i] = X[c][i] - l * X[c][k];
+      if (LAST) b[i] = b[i] - l * b[k];
+    }
+  }
+  lu_panel<M, BLOCK, C0, CB, LAST, !LAST>(ar, jac, rowoff, X, b, rinv, ok);
+  if constexpr (!LAST) {
+    lu_panels_from<M, BLOCK, PI + 1>(ar, jac, rowoff, b, ok);
+  } else {
+    // back substitution: U of this panel from the registers, U of the earlier ones from shared memory
+#pragma unroll
+    for (int i = M - 1; i >= 0; i--) {
+      double s = b[i];
+#pragma unroll
+      for (int j = i + 1; j < M; j++) {
+        const int jc = j >= C0 ? j - C0 : 0;
+        if (j >= C0) s = s - X[jc][i] * b[j];
+        else s = s - jac.at(rowoff[i], j) * b[j];
+      }
+      const int ic = i >= C0 ? i - C0 : 0;
+      if (i >= C0) b[i] = s * rinv[ic];
+      else b[i] = s * jac.at(rowoff[i], i);
+    }
+  }
+}
+
+template <int M, int BLOCK, class A>
+__device__ __forceinline__ bool lu_solve_panels(A &ar, const JacView<M, BLOCK> &jac, double (&b)[M]) {
+  int rowoff[M];
+#pragma unroll
+  for (int i = 0; i < M; i++) rowoff[i] = JacView<M, BLOCK>::row(i);
+  bool ok = true;
+  lu_panels_from<M, BLOCK, 0>(ar, jac, rowoff, b, ok);
+  return ok;
+}
+
+#ifndef GRIM_LU_PANELS
+#define GRIM_LU_PANELS 0
+#endif
+
 // eq 25 (L230): minimiser of the quadratic through f(0), f'(0) = -2 f(0), f(lam)
 template <class A>
 __device__ __forceinline__ double linesearch_lambda(A &ar, double f0, double flam, double lam) {
@@ -269,7 +447,11 @@ __device__ __forceinline__ double newton_zone(A &ar, const Prob &prob, const Sol
     double dP[M];
 #pragma unroll
     for (int v = 0; v < M; v++) dP[v] = -R0[U::prim(v)];
+#if GRIM_LU_PANELS
+    bool ok = lu_solve_panels<M, BLOCK>(ar, jac, dP);
+#else
     bool ok = lu_solve<M, BLOCK>(ar, jac, dP);
+#endif
     if (singular || !ok) {
       st |= ST_SINGULAR;
       break;
