@@ -161,12 +161,21 @@ static double sound_speed2(const og_model *m, const double *P) {
   return m->gam * pressure(m, P) / (P[OG_RHO] + m->gam * P[OG_UU]);
 }
 
+/* Closure: thermal diffusivity chi and kinematic viscosity nu of state P.  OG_CLOSURE_CS2TAU: chi = phi cs^2 tau_R,
+ * nu = psi cs^2 tau_R (L299).  OG_CLOSURE_CONST: constants chi = phi, nu = psi, as the anisotropic-conduction test
+ * prescribes ("the thermal diffusivity chi = 0.01", L566). */
+static void closure(const og_model *m, double tau, double cs2, double *chi, double *nu) {
+  if (m->closure == OG_CLOSURE_CONST) { *chi = m->phi; *nu = m->psi; return; }
+  *chi = m->phi * cs2 * tau;
+  *nu = m->psi * cs2 * tau;
+}
+
 /* eqs 41-42 (L291-293): q~ = q sqrt(tau/(chi rho Theta^2)), dP~ = dP sqrt(tau/(nu rho Theta)); closure of
  * the same state P (C-4) */
 void og_rescale_factors(const og_model *m, double tau, const double *P, double *fq, double *fdp) {
   double cs2 = sound_speed2(m, P);
-  double chi = m->phi * cs2 * tau;
-  double nu = m->psi * cs2 * tau;
+  double chi, nu;
+  closure(m, tau, cs2, &chi, &nu);
   double Th = temperature(m, P);
   *fq = sqrt(tau / (chi * P[OG_RHO] * Th * Th));
   *fdp = sqrt(tau / (nu * P[OG_RHO] * Th));
@@ -255,7 +264,8 @@ static double vmax2_state(const og_model *m, double tau, const double *P, const 
   double va2 = s->bsq / (rho + m->gam * u + s->bsq);       /* eq 44 */
   double cst2 = cs2;
   if (m->nvar == 10) {
-    double chi = m->phi * cs2 * tau, nu = m->psi * cs2 * tau;
+    double chi, nu;
+    closure(m, tau, cs2, &chi, &nu);
     double vq2 = (m->gam - 1.0) * chi / tau;               /* eq 47 */
     double vdp2 = 4.0 * nu / (3.0 * tau);                  /* eq 48 */
     cst2 = 0.5 * (cs2 + vq2 + sqrt(cs2 * cs2 + vq2 * vq2)) + vdp2;  /* eq 46 */
@@ -472,7 +482,8 @@ static void emhd_coefficients(const og_model *m, const og_geom *g, double tau, c
   c->ThE = temperature(m, PE);
   c->utE = sE->ucon[0];
   double cs2 = sound_speed2(m, PE);
-  double chi = m->phi * cs2 * tau, nu = m->psi * cs2 * tau;
+  double chi, nu;
+  closure(m, tau, cs2, &chi, &nu);
   c->rhochi = PE[OG_RHO] * chi;
   c->rhonu3 = 3.0 * PE[OG_RHO] * nu;
   og_rescale_factors(m, tau, PE, &c->fqE, &c->fdE);
@@ -526,7 +537,7 @@ static inline int64_t zidx(const og_grid *g, int i, int j, int k) {
 og_grid *og_grid_create(const og_grid_desc *d) {
   og_grid *g = (og_grid *)calloc(1, sizeof(og_grid));
   g->d = *d;
-  g->m.nvar = d->nvar; g->m.gam = d->gam; g->m.phi = d->phi; g->m.psi = d->psi;
+  g->m.nvar = d->nvar; g->m.gam = d->gam; g->m.phi = d->phi; g->m.psi = d->psi; g->m.closure = d->closure;
   g->s.fd_eps = d->fd_eps; g->s.eps_bt = d->eps_bt; g->s.atol = d->atol; g->s.rtol = d->rtol;
   g->s.kmax = d->kmax; g->s.lsmax = d->lsmax;
   g->n[0] = d->n1; g->n[1] = d->n2; g->n[2] = d->n3;

@@ -45,6 +45,7 @@ enum { OG_MINMOD = 0, OG_MP5 = 1 };
 enum { OG_LLF = 0, OG_HLLE = 1 };
 enum { OG_BC_PERIODIC = 0, OG_BC_OUTFLOW = 1, OG_BC_REFLECT_POLAR = 2, OG_BC_NONE = 3 };
 enum { OG_TAU_CONST = 0, OG_TAU_R32 = 1 };
+enum { OG_CLOSURE_CS2TAU = 0, OG_CLOSURE_CONST = 1 };
 
 /* status word per zone */
 enum { OG_ST_CONVERGED = 1, OG_ST_KMAX = 2, OG_ST_LS_EXHAUSTED = 4,
@@ -64,6 +65,7 @@ typedef struct {
   int32_t nvar;       /* 8 ideal GRMHD, 10 EMHD */
   double  gam;        /* adiabatic index (L248) */
   double  phi, psi;   /* closure chi = phi cs^2 tau_R, nu = psi cs^2 tau_R (L299) */
+  int32_t closure;    /* OG_CLOSURE_CS2TAU (L299) | OG_CLOSURE_CONST: chi = phi, nu = psi constants (L566) */
 } og_model;
 
 /* solver parameters (eqs 20-25; C-2, C-14, C-16) */
@@ -89,6 +91,7 @@ typedef struct {
   int32_t kmax, lsmax;
   double  cfl;
   int32_t flux_ct;    /* != 0: flux-CT averaging of the magnetic-field fluxes (PAPER.md 4.2, L327-335) */
+  int32_t closure;    /* OG_CLOSURE_* */
   int32_t reduced;    /* != 0: the paper's own split (L148 "equations without implicitly coupled source terms are
                          treated explicitly", L643 "5 x 5 ... as opposed to a 7 x 7 Jacobian"): B^i advanced
                          explicitly, Newton on the nvar-3 other primitives */

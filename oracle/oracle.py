@@ -20,6 +20,7 @@ MINMOD, MP5 = 0, 1
 LLF, HLLE = 0, 1
 BC_PERIODIC, BC_OUTFLOW, BC_REFLECT_POLAR, BC_NONE = 0, 1, 2, 3
 TAU_CONST, TAU_R32 = 0, 1
+CLOSURE_CS2TAU, CLOSURE_CONST = 0, 1
 ST_CONVERGED, ST_KMAX, ST_LS_EXHAUSTED, ST_SINGULAR, ST_NONFINITE = 1, 2, 4, 8, 16
 
 
@@ -29,7 +30,8 @@ class Geom(C.Structure):
 
 
 class Model(C.Structure):
-    _fields_ = [("nvar", C.c_int32), ("gam", C.c_double), ("phi", C.c_double), ("psi", C.c_double)]
+    _fields_ = [("nvar", C.c_int32), ("gam", C.c_double), ("phi", C.c_double), ("psi", C.c_double),
+                ("closure", C.c_int32)]
 
 
 class Solver(C.Structure):
@@ -44,7 +46,8 @@ class GridDesc(C.Structure):
                 ("riemann", C.c_int32), ("gam", C.c_double), ("phi", C.c_double), ("psi", C.c_double),
                 ("tau_mode", C.c_int32), ("tau", C.c_double),
                 ("fd_eps", C.c_double), ("eps_bt", C.c_double), ("atol", C.c_double), ("rtol", C.c_double),
-                ("kmax", C.c_int32), ("lsmax", C.c_int32), ("cfl", C.c_double), ("flux_ct", C.c_int32), ("reduced", C.c_int32)]
+                ("kmax", C.c_int32), ("lsmax", C.c_int32), ("cfl", C.c_double), ("flux_ct", C.c_int32),
+                ("closure", C.c_int32), ("reduced", C.c_int32)]
 
 
 class StepStats(C.Structure):
@@ -159,8 +162,8 @@ def geom_arrays(g):
             np.array([[g.gcon[i][j] for j in range(4)] for i in range(4)]), g.sqrtmg, g.alpha)
 
 
-def model(nvar=10, gam=4.0 / 3.0, phi=1.0, psi=1.0):
-    return Model(nvar, gam, phi, psi)
+def model(nvar=10, gam=4.0 / 3.0, phi=1.0, psi=1.0, closure=0):
+    return Model(nvar, gam, phi, psi, closure)
 
 
 def solver(fd_eps=4e-8, eps_bt=1e-4, atol=0.0, rtol=1e-12, kmax=30, lsmax=8):
@@ -309,10 +312,12 @@ class Grid:
     def __init__(self, n1, n2=1, n3=1, ng=3, dim=2, xstart=(0, 0, 0), xend=(1, 1, 1),
                  bc=BC_PERIODIC, nvar=10, recon=MINMOD, limiter_theta=1.0, gam=4.0 / 3.0, phi=1.0, psi=1.0,
                  tau_mode=TAU_CONST, tau=1.0, fd_eps=4e-8, eps_bt=1e-4, atol=0.0, rtol=1e-14, kmax=8,
-                 lsmax=5, cfl=0.5, metric=MINKOWSKI, metric_params=(), flux_ct=False, reduced=False, riemann=0):
+                 lsmax=5, cfl=0.5, metric=MINKOWSKI, metric_params=(), flux_ct=False, reduced=False, riemann=0,
+                 closure=0):
         d = GridDesc()
         d.flux_ct = 1 if flux_ct else 0
         d.reduced = 1 if reduced else 0
+        d.closure = closure
         d.n1, d.n2, d.n3, d.ng, d.dim = n1, n2, n3, ng, dim
         for a in range(3):
             d.xstart[a], d.xend[a] = float(xstart[a]), float(xend[a])

@@ -99,6 +99,33 @@ struct JacView {
   static __device__ __forceinline__ constexpr int row(int r) { return r * N * BLOCK; }
 };
 
+// Structure of the Jacobian that holds for both residuals (problems.cuh) whatever the state: entry (row, col) is
+// (R_row(P_eps,col) - R_row(P)) * ih with R_row(P_eps,col) the SAME bits as R_row(P) -- exactly +0 * ih -- when
+// R_row does not read primitive col:
+//   * row B^i reads B^i only (U_{B^i} = sqrt(-g) B^i, no source; eq 30, O-3),
+//   * row rho reads rho and u~^i only (U_rho = sqrt(-g) rho u^t),
+//   * rows q, dP read rho, u (rescale factors, Theta), u~^i and their own primitive; not B^i (the bhat of the source
+//     terms is P_E's, O-8), not each other.
+// Those 41 of the 100 entries are stored as that signed zero without evaluating the row (the perturbed evaluation
+// then skips the row altogether), and the B rows, which the structured solve below never reads, are not stored.
+template <int N>
+__host__ __device__ constexpr bool jac_zero(int row, int col) {
+  if (row >= B1 && row <= B3) return col != row;
+  if (row == RHO) return col == UU || (col >= B1 && col <= B3) || col >= QQ;
+  if (row >= QQ) return (col >= B1 && col <= B3) || (col >= QQ && col != row);
+  return false;
+}
+#ifndef GRIM_JAC_STRUCT
+#define GRIM_JAC_STRUCT 1
+#endif
+// full solves of both problems use the structure; the reduced solve has no B rows and keeps the general path
+template <int N, bool RED>
+__host__ __device__ constexpr bool use_structure() { return GRIM_JAC_STRUCT && !RED; }
+
+__device__ __forceinline__ double zero_times(double ih) {  // (+0) * ih for finite ih
+  return __hiloint2double(__double2hiint(ih) & 0x80000000, 0);
+}
+
 // One finite-difference column (eqs 22-23): J[:,j] = (R(P_eps,j) - R0) / (P_eps,j - P_j)
 // (column S of the M x M Jacobian: unknown S = primitive prim(S))
 template <int S, int N, bool RED, int BLOCK, class A, class Prob>
@@ -107,6 +134,7 @@ __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverP
                                           const JacView<Unknowns<N, RED>::M, BLOCK> &jac, bool &singular) {
   using U = Unknowns<N, RED>;
   constexpr int J = U::prim(S);
+  constexpr bool STRUCT = use_structure<N, RED>();
   double pj = (fabs(P[J]) < 5.0 * sp.fd_eps) ? sp.fd_eps : (1.0 + sp.fd_eps) * P[J];
   double h = pj - P[J];
   if (h == 0.0) singular = true;
@@ -114,8 +142,14 @@ __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverP
   double Rt[N];
   eval_column<J, N>(ar, prob, P, pj, base, Rt);
 #pragma unroll
-  for (int i = 0; i < U::M; i++)
-    jac.at(JacView<U::M, BLOCK>::row(i), S) = (Rt[U::prim(i)] - R0[U::prim(i)]) * ih;
+  for (int i = 0; i < U::M; i++) {
+    const int row = U::prim(i);
+    if (GRIM_JAC_STRUCT && jac_zero<N>(row, J)) {
+      if (!(STRUCT && row >= B1 && row <= B3)) jac.at(JacView<U::M, BLOCK>::row(i), S) = zero_times(ih);
+    } else {
+      jac.at(JacView<U::M, BLOCK>::row(i), S) = (Rt[row] - R0[row]) * ih;
+    }
+  }
 }
 
 // Order in which the (independent) columns are evaluated: first those that reuse every piece of the unperturbed
@@ -412,6 +446,150 @@ __device__ __forceinline__ bool lu_solve_panels(A &ar, const JacView<M, BLOCK> &
 #define GRIM_LU_PANELS 0
 #endif
 
+// ---------------------------------------------------------------------------------------------------------
+// The factorisation of the full N x N Jacobian with its structure (jac_zero) used.  The B rows are zero in the
+// columns of rho, u, u~^i, so in the elimination steps k = 0..4 they are never the pivot (a zero is never the
+// first maximal |x_i| unless every candidate is zero, which is the singular exit either way), their
+// multipliers are exact zeros and their updates x - 0 * x_k are no-ops: steps 0..4 run on the N - 3 other rows
+// ("active": positions 0..4 and, for EMHD, 8, 9) and leave the B rows in positions 5..7 as they were stored.
+//   A  columns 0..4, left-looking, one column of the active rows in registers (as lu_solve above);
+//   B  columns 5..N-1 and the right-hand side: active rows updated by the pivots 0..4 (G columns at a time share
+//      one load of the multipliers); rows 0..4 of the result are final entries of U and go to shared memory;
+//   C  the trailing (N-5) x (N-5) block -- B rows: diagonal only; positions 8, 9: from B -- is factorised and
+//      solved in registers with full partial pivoting (lu_panel), so a B row losing the pivot to a q / dP row
+//      is handled like any other exchange;
+//   D  back substitution of the unknowns 4..0.
+// Every element receives the same updates in the same order as in og_lu_solve / lu_solve except those skipped
+// no-ops, which can change nothing but the sign of an exact zero.
+// ---------------------------------------------------------------------------------------------------------
+#ifndef GRIM_LU_GROUP
+#define GRIM_LU_GROUP 5
+#endif
+template <int N, int BLOCK, class A>
+__device__ __forceinline__ bool lu_solve_structured(A &ar, const JacView<N, BLOCK> &jac, double (&b)[N]) {
+  constexpr int NA = N - 3;   // active rows
+  constexpr int NT = N - 5;   // trailing block
+  constexpr int G = GRIM_LU_GROUP;
+  int ro[NA];
+  double ba[NA];
+#pragma unroll
+  for (int a = 0; a < NA; a++) {
+    const int pos = a < 5 ? a : a + 3;
+    ro[a] = JacView<N, BLOCK>::row(pos);
+    ba[a] = b[pos];
+  }
+  bool ok = true;
+  // A
+#pragma unroll
+  for (int j = 0; j < 5; j++) {
+    double x[NA];
+#pragma unroll
+    for (int a = 0; a < NA; a++) x[a] = jac.at(ro[a], j);
+#pragma unroll
+    for (int k = 0; k < j; k++) {
+#pragma unroll
+      for (int a = k + 1; a < NA; a++) {
+        const double l = jac.at(ro[a], k);
+        x[a] = x[a] - l * x[k];
+      }
+    }
+    int p = j;
+    double xp = x[j], amax = fabs(x[j]);
+#pragma unroll
+    for (int a = j + 1; a < NA; a++) {
+      const double v = fabs(x[a]);
+      const bool gt = v > amax;
+      amax = gt ? v : amax;
+      xp = gt ? x[a] : xp;
+      p = gt ? a : p;
+    }
+    ok = ok && (amax > 0.0) && isfinite(amax);
+    const double r = ar.rcp(xp);
+    const int roj = ro[j];
+    int rop = roj;
+#pragma unroll
+    for (int a = j + 1; a < NA; a++) rop = (p == a) ? ro[a] : rop;
+#pragma unroll
+    for (int a = 0; a < j; a++) jac.at(ro[a], j) = x[a];
+#pragma unroll
+    for (int a = j; a < NA; a++) jac.at(ro[a], j) = x[a] * r;
+    jac.at(rop, j) = r;
+#pragma unroll
+    for (int a = j + 1; a < NA; a++) ro[a] = (p == a) ? roj : ro[a];
+    ro[j] = rop;
+    swap_positions<NA>(ba, j, p);
+  }
+  // B
+  double T[NT][NT], t[NT];
+#pragma unroll
+  for (int c0 = 5; c0 < N; c0 += G) {
+    double x[G][NA];
+#pragma unroll
+    for (int g = 0; g < G; g++)
+#pragma unroll
+      for (int a = 0; a < NA; a++)
+        if (c0 + g < N) x[g][a] = jac.at(ro[a], c0 + g);
+    const bool with_rhs = (c0 + G >= N);
+#pragma unroll
+    for (int k = 0; k < 5; k++) {
+#pragma unroll
+      for (int a = k + 1; a < NA; a++) {
+        const double l = jac.at(ro[a], k);
+#pragma unroll
+        for (int g = 0; g < G; g++)
+          if (c0 + g < N) x[g][a] = x[g][a] - l * x[g][k];
+        if (with_rhs) ba[a] = ba[a] - l * ba[k];
+      }
+    }
+#pragma unroll
+    for (int g = 0; g < G; g++) {
+      if (c0 + g < N) {
+#pragma unroll
+        for (int a = 0; a < 5; a++) jac.at(ro[a], c0 + g) = x[g][a];
+#pragma unroll
+        for (int a = 5; a < NA; a++) T[c0 + g - 5][a - 2] = x[g][a];
+      }
+    }
+  }
+  // C
+#pragma unroll
+  for (int c = 0; c < NT; c++)
+#pragma unroll
+    for (int i = 0; i < 3; i++) T[c][i] = (c == i) ? jac.at(JacView<N, BLOCK>::row(5 + i), 5 + i) : 0.0;
+#pragma unroll
+  for (int i = 0; i < 3; i++) t[i] = b[5 + i];
+#pragma unroll
+  for (int a = 5; a < NA; a++) t[a - 2] = ba[a];
+  {
+    int rdummy[NT];
+#pragma unroll
+    for (int i = 0; i < NT; i++) rdummy[i] = 0;
+    double tinv[NT];
+    const JacView<NT, BLOCK> nojac{jac.base};
+    lu_panel<NT, BLOCK, 0, NT, true, false>(ar, nojac, rdummy, T, t, tinv, ok);
+#pragma unroll
+    for (int i = NT - 1; i >= 0; i--) {
+      double sacc = t[i];
+#pragma unroll
+      for (int j = i + 1; j < NT; j++) sacc = sacc - T[j][i] * t[j];
+      t[i] = sacc * tinv[i];
+    }
+  }
+  // D
+#pragma unroll
+  for (int a = 4; a >= 0; a--) {
+    double sacc = ba[a];
+#pragma unroll
+    for (int j = a + 1; j < N; j++) sacc = sacc - jac.at(ro[a], j) * (j < 5 ? ba[j] : t[j - 5]);
+    ba[a] = sacc * jac.at(ro[a], a);
+  }
+#pragma unroll
+  for (int i = 0; i < 5; i++) b[i] = ba[i];
+#pragma unroll
+  for (int i = 5; i < N; i++) b[i] = t[i - 5];
+  return ok;
+}
+
 // eq 25 (L230): minimiser of the quadratic through f(0), f'(0) = -2 f(0), f(lam)
 template <class A>
 __device__ __forceinline__ double linesearch_lambda(A &ar, double f0, double flam, double lam) {
@@ -447,11 +625,16 @@ __device__ __forceinline__ double newton_zone(A &ar, const Prob &prob, const Sol
     double dP[M];
 #pragma unroll
     for (int v = 0; v < M; v++) dP[v] = -R0[U::prim(v)];
+    bool ok;
+    if constexpr (use_structure<N, RED>()) {
+      ok = lu_solve_structured<M, BLOCK>(ar, jac, dP);
+    } else {
 #if GRIM_LU_PANELS
-    bool ok = lu_solve_panels<M, BLOCK>(ar, jac, dP);
+      ok = lu_solve_panels<M, BLOCK>(ar, jac, dP);
 #else
-    bool ok = lu_solve<M, BLOCK>(ar, jac, dP);
+      ok = lu_solve<M, BLOCK>(ar, jac, dP);
 #endif
+    }
     if (singular || !ok) {
       st |= ST_SINGULAR;
       break;

@@ -190,16 +190,31 @@ def test_kerr_timestep_fixed_count_matches_oracle(nvar, recon):
             assert so.max_resnorm[s] < 1e-14 and sc.max_resnorm[s] < 1e-14      # at the round-off floor
     err = rel_err_per_primitive(dP.cpu().numpy(), Po, go.interior, gam=4.0 / 3.0)
     assert err.max() <= 1e-10, err
+    # SURVEY 8(d)'s literal measure (|A-B| / max(|B|, 1e-12 max_z|B_v|), no natural scale for q, dP): met by every
+    # primitive but q and dP, which pass through zero inside the domain while their relaxation targets (eqs 37-38) are
+    # differences of terms of the natural size rho Theta^{3/2}, P_g -- so a 1e-12 difference of the connection
+    # coefficients moves them by ~1e-12 of THAT size whatever their own magnitude.  Recorded bound (DESIGN.md
+    # "Tolerances" prints the measured values): three steps stay below 1e-7 of max(|q|, floor) even there.
+    lit = rel_err_per_primitive(dP.cpu().numpy(), Po, go.interior)
+    assert lit[:8].max() <= 1e-10, lit
+    if nvar == 10:
+        print("literal-measure error of q, dP after 3 steps with device geometry:", lit[8:])
+        assert lit[8:].max() <= 1e-7, lit
 
 
-def test_kerr_timestep_tolerance_mode_counts():
-    """Same run with a convergence tolerance (rtol = 1e-13) that cuts through the post-iteration-2 residual
-    distribution (no gap exists on this grid): primitives still agree to 1e-10 and the per-zone iteration counts
-    agree except for threshold flips caused by the last-bit geometry differences -- at most one iteration apart,
-    in well under 1 % of the zones (normally none)."""
+@pytest.mark.parametrize("tables", ["oracle", "device"])
+def test_kerr_timestep_tolerance_mode_counts(tables):
+    """One stage with a convergence tolerance (rtol = 1e-13) that cuts through the post-iteration-2 residual
+    distribution (no gap exists on this grid).  With the oracle's geometry tables the per-zone iteration counts,
+    statuses, residual norms and primitives are IDENTICAL (north star).  With the library's own geometry precompute
+    the tables differ from the oracle's in the last bits (device libm vs glibc: a0's parity is 1e-12 per tensor), so
+    a zone whose residual sits within that distance of the threshold may stop one iteration apart -- counted, and
+    bounded to well under 1 % of the zones -- while the primitives still agree to 1e-10."""
     import torch
     gk = dict(KERR)
     go, gc = oracle_grid(gk), cuda_grid(gk)
+    if tables == "oracle":
+        gc.set_metric_tables(*go.geometry_tables())
     P0 = kerr_state(go, 4)
     dt = go.choose_dt(P0)
     Co, Go, _ = go.stage_prepare(P0, P0, 0.5 * dt)
@@ -211,6 +226,13 @@ def test_kerr_timestep_tolerance_mode_counts():
     drn, dst, dit = gc.zeros(), gc.zeros(dtype=torch.int32), gc.zeros(dtype=torch.int32)
     assert gc.newton_step(dPn, dPn, None, None, 0.5 * dt, 0, dP, drn, dst, dit) == 0
     ito, itc = go.interior(it), go.interior(dit.cpu().numpy())
+    assert len(np.unique(ito)) > 1          # the tolerance does cut the distribution: counts are not all equal
+    if tables == "oracle":
+        assert np.array_equal(itc, ito)
+        assert np.array_equal(go.interior(dst.cpu().numpy()), go.interior(st))
+        assert np.array_equal(go.interior(drn.cpu().numpy()), go.interior(rn))
+        assert np.array_equal(go.interior(dP.cpu().numpy()), go.interior(Po))
+        return
     diff = ito != itc
     assert diff.mean() < 0.01 and (abs(ito - itc) <= 1).all(), (diff.sum(), ito.size)
     assert (go.interior(st) & og.ST_CONVERGED).all() and (go.interior(dst.cpu().numpy()) & og.ST_CONVERGED).all()
