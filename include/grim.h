@@ -54,6 +54,7 @@ enum { GRIM_LLF = 0, GRIM_HLLE = 1 };
 enum { GRIM_BC_PERIODIC = 0, GRIM_BC_OUTFLOW = 1, GRIM_BC_REFLECT_POLAR = 2, GRIM_BC_NONE = 3 };
 /* damping time scale tau_R: constant, or r^{3/2} (C-11) */
 enum { GRIM_TAU_CONST = 0, GRIM_TAU_R32 = 1 };
+enum { GRIM_CLOSURE_CS2TAU = 0, GRIM_CLOSURE_CONST = 1 };
 
 /* per-zone status word */
 enum {
@@ -96,6 +97,10 @@ typedef struct {
                                grim_newton_step / grim_newton_solve / grim_timestep runs on the other N - 3 primitives
                                (5 x 5 / 7 x 7 Jacobian); ||R||, the tolerance and the status refer to those rows.
                                0 (default): all N primitives are unknowns (BASELINE.json).                           */
+  int32_t closure;          /* GRIM_CLOSURE_CS2TAU (0, default): chi = phi cs^2 tau_R, nu = psi cs^2 tau_R (L299).
+                               GRIM_CLOSURE_CONST: phi and psi ARE the thermal diffusivity chi and the kinematic
+                               viscosity nu, constants, as the anisotropic-conduction test prescribes (L566:
+                               "the thermal diffusivity chi = 0.01").                                                */
 } grim_grid_desc;
 
 typedef struct {

@@ -30,7 +30,8 @@ class GridDesc(C.Structure):
                 ("tau_mode", C.c_int32), ("tau", C.c_double),
                 ("fd_eps", C.c_double), ("eps_bt", C.c_double), ("atol", C.c_double), ("rtol", C.c_double),
                 ("kmax", C.c_int32), ("lsmax", C.c_int32), ("cfl", C.c_double),
-                ("device", C.c_int32), ("stream", C.c_void_p), ("flux_ct", C.c_int32), ("reduced_solve", C.c_int32)]
+                ("device", C.c_int32), ("stream", C.c_void_p), ("flux_ct", C.c_int32), ("reduced_solve", C.c_int32),
+                ("closure", C.c_int32)]
 
 
 class StepStats(C.Structure):
@@ -127,7 +128,8 @@ class Grid:
     def __init__(self, n1, n2=1, n3=1, ng=3, dim=2, xstart=(0.0, 0.0, 0.0), xend=(1.0, 1.0, 1.0), bc=BC_PERIODIC,
                  model=EMHD, recon=MINMOD, limiter_theta=1.0, gamma=4.0 / 3.0, phi=1.0, psi=1.0, tau_mode=TAU_CONST,
                  tau=1.0, fd_eps=4e-8, eps_bt=1e-4, atol=0.0, rtol=1e-14, kmax=8, lsmax=5, cfl=0.5,
-                 metric=MINKOWSKI, metric_params=(), device=0, stream=None, flux_ct=False, reduced=False, riemann=LLF):
+                 metric=MINKOWSKI, metric_params=(), device=0, stream=None, flux_ct=False, reduced=False, riemann=LLF,
+                 closure=0):
         import torch
         self.torch = torch
         d = GridDesc()
@@ -142,6 +144,7 @@ class Grid:
         d.device = device
         d.flux_ct = 1 if flux_ct else 0
         d.reduced_solve = 1 if reduced else 0
+        d.closure = closure
         if stream is None and torch.cuda.is_available():
             stream = torch.cuda.current_stream(device).cuda_stream
         d.stream = stream

@@ -179,6 +179,8 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   if (!(d->gamma > 1.0)) return fail(c, GRIM_EINVAL, "adiabatic index must exceed 1");
   if (!(d->limiter_theta >= 1.0 && d->limiter_theta <= 2.0)) return fail(c, GRIM_EINVAL, "limiter_theta outside [1,2]");
   if (!(d->fd_eps > 0.0) || d->kmax < 0 || d->lsmax < 0) return fail(c, GRIM_EINVAL, "bad solver parameters");
+  if (d->closure != GRIM_CLOSURE_CS2TAU && d->closure != GRIM_CLOSURE_CONST)
+    return fail(c, GRIM_EINVAL, "unknown closure");
   if (d->model == GRIM_EMHD && !(d->tau_mode == GRIM_TAU_R32 || d->tau > 0.0))
     return fail(c, GRIM_EINVAL, "tau_R must be positive");
 
@@ -223,6 +225,7 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   gv.m.gm1 = d->gamma - 1.0;
   gv.m.phi = d->phi;
   gv.m.psi = d->psi;
+  gv.m.closure = d->closure ? 1 : 0;
   gv.tau_const = d->tau;
   gv.sp.fd_eps = d->fd_eps;
   gv.sp.eps_bt = d->eps_bt;

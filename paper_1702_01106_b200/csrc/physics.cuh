@@ -23,7 +23,15 @@ enum { RHO = 0, UU = 1, U1 = 2, U2 = 3, U3 = 4, B1 = 5, B2 = 6, B3 = 7, QQ = 8, 
 struct ModelParams {
   double gam, gm1;   // adiabatic index, gam - 1 (L248)
   double phi, psi;   // closure coefficients (L299)
+  int closure;       // 0: chi = phi cs^2 tau, nu = psi cs^2 tau (L299); 1: chi = phi, nu = psi constants (L566)
 };
+
+// thermal diffusivity and kinematic viscosity of a state with sound speed cs2 (L299; constant variant L566)
+__device__ __forceinline__ void closure_coeffs(const ModelParams &m, double cs2, double tau, double &chi, double &nu) {
+  const double c = m.phi * cs2 * tau, n = m.psi * cs2 * tau;
+  chi = m.closure ? m.phi : c;
+  nu = m.closure ? m.psi : n;
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // Geometry of one evaluation point.  Minkowski is a compile-time constant; a general stationary metric is a
@@ -157,8 +165,8 @@ __device__ __forceinline__ void thermo_state(A &ar, const ModelParams &m, double
   if constexpr (N == 10) {
     t.Th = ar.div(t.Pg, rho);
     double cs2 = ar.div(m.gam * t.Pg, rho + m.gam * u);
-    double chi = m.phi * cs2 * tau;
-    double nu = m.psi * cs2 * tau;
+    double chi, nu;
+    closure_coeffs(m, cs2, tau, chi, nu);
     t.fq = ar.sqrt(ar.div(tau, chi * rho * t.Th * t.Th));
     t.fdp = ar.sqrt(ar.div(tau, nu * rho * t.Th));
   } else {
@@ -244,7 +252,8 @@ __device__ __forceinline__ double vmax2(A &ar, const ModelParams &m, double tau,
   double va2 = ar.div_z(bsq, rho + m.gam * u + bsq);
   double cst2 = cs2;
   if constexpr (N == 10) {
-    double chi = m.phi * cs2 * tau, nu = m.psi * cs2 * tau;
+    double chi, nu;
+    closure_coeffs(m, cs2, tau, chi, nu);
     double vq2 = ar.div(m.gm1 * chi, tau);
     double vdp2 = ar.div(4.0 * nu, 3.0 * tau);
     cst2 = 0.5 * (cs2 + vq2 + ar.sqrt(cs2 * cs2 + vq2 * vq2)) + vdp2;

@@ -56,7 +56,8 @@ struct StageProblem {
       ThE = pe.th.Th;
       utE = pe.v.ucon[0];
       double cs2 = sound_speed2(ar, m, PE[RHO], PE[UU]);
-      double chi = m.phi * cs2 * tau_, nu = m.psi * cs2 * tau_;
+      double chi, nu;
+      closure_coeffs(m, cs2, tau_, chi, nu);
       nrhochi = -(PE[RHO] * chi);
       rhonu3 = 3.0 * PE[RHO] * nu;
       fqE = pe.th.fq;

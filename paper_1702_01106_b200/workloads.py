@@ -140,3 +140,24 @@ def firehose(n=64, alpha=1e-6):
     P[3] = 0.1628 * alpha * np.sin(2 * np.pi * X1)
     P[6] = 0.9867 * alpha * np.cos(2 * np.pi * X1)
     return grid, P
+
+
+def conduction(n=64, A=0.2, R2=0.005, B0=1e-4, k=4, chi=0.01, nu=0.01, tau=0.1):
+    """Anisotropic-conduction test of the paper (L538-572, eqs 53-57): 2-D Minkowski, periodic on [0,1]^2, EMHD with
+    the CONSTANT thermal diffusivity chi = 0.01 and tau_R = 0.1 the paper prescribes (closure = 1: chi = phi, nu = psi
+    as constants; the paper gives no viscosity for this test, reading C-24: nu = chi), gamma = 4/3:
+    rho = 1 - A exp(-r^2/R^2) about the centre of the box, u = 1 (pressure equilibrium), fluid at rest,
+    B^1 = B0, B^2 = B0 sin(2 pi k x^1), q = dP = 0.  Returns (grid description, P)."""
+    grid = dict(n1=n, n2=n, n3=1, ng=3, dim=2, xstart=(0.0, 0.0, 0.0), xend=(1.0, 1.0, 1.0), nvar=10, recon=1,
+                limiter_theta=2.0, gam=4.0 / 3.0, phi=chi, psi=nu, closure=1, tau=tau, rtol=1e-13, kmax=10, lsmax=5,
+                cfl=0.5)
+    X1, X2, _ = padded_centres((n, n, 1), (3, 3, 0), grid["xstart"], grid["xend"])
+    # periodic images of the blob are exp(-1/0.005) away: the nearest image only
+    d1 = (X1 - 0.5 + 0.5) % 1.0 - 0.5
+    d2 = (X2 - 0.5 + 0.5) % 1.0 - 0.5
+    P = np.zeros((10,) + X1.shape)
+    P[0] = 1.0 - A * np.exp(-(d1 * d1 + d2 * d2) / R2)
+    P[1] = 1.0
+    P[5] = B0
+    P[6] = B0 * np.sin(2 * np.pi * k * X1)
+    return grid, P

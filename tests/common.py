@@ -16,7 +16,7 @@ def oracle_grid(gk, **over):
                    kmax=k.get("kmax", 8), lsmax=k.get("lsmax", 5), cfl=k.get("cfl", 0.5),
                    metric=k.get("metric", 0), metric_params=k.get("metric_params", ()),
                    flux_ct=k.get("flux_ct", False), reduced=k.get("reduced", False),
-                   riemann=k.get("riemann", 0))
+                   riemann=k.get("riemann", 0), closure=k.get("closure", 0))
 
 
 def cuda_grid(gk, **over):
@@ -31,7 +31,8 @@ def cuda_grid(gk, **over):
                    eps_bt=k.get("eps_bt", 1e-4), atol=k.get("atol", 0.0), rtol=k.get("rtol", 1e-14),
                    kmax=k.get("kmax", 8), lsmax=k.get("lsmax", 5), cfl=k.get("cfl", 0.5),
                    metric=k.get("metric", 0), metric_params=k.get("metric_params", ()),
-                   flux_ct=k.get("flux_ct", False), reduced=k.get("reduced", False), riemann=k.get("riemann", 0))
+                   flux_ct=k.get("flux_ct", False), reduced=k.get("reduced", False), riemann=k.get("riemann", 0),
+                   closure=k.get("closure", 0))
 
 
 def to_dev(a, dtype=None):

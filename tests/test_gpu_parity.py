@@ -349,6 +349,26 @@ def test_firehose_workload_matches_oracle():
     assert abs(go.interior(Pc)[6]).max() > abs(go.interior(P0)[6]).max()
 
 
+def test_conduction_workload_matches_oracle():
+    """The paper's anisotropic-conduction test (L538-572, eqs 53-57) with the constant closure
+    chi = 0.01, tau_R = 0.1 (L566) at 64^2: sixty steps bit-identical to the oracle, the per-stage Newton iteration
+    histograms, backtrack and non-convergence counts and the largest residual norm equal bin by bin at every step, and
+    the histogram is non-trivial (strong q relaxation: counts spread over several bins, unlike configs 1 / 3)."""
+    from paper_1702_01106_b200 import workloads
+    gk, P0 = workloads.conduction(n=64)
+    go = oracle_grid(gk)
+    go.fill_ghosts(P0)
+    dt = go.choose_dt(P0)
+    go, Po, Pc, stats = run_steps(gk, P0, 60, dt)
+    check_stats(stats)
+    assert np.array_equal(go.interior(Pc), go.interior(Po))
+    hist = np.zeros(16, dtype=np.int64)
+    for so, _ in stats:
+        hist += np.array(so.iters_hist[0]) + np.array(so.iters_hist[1])
+    assert (hist > 0).sum() >= 2, hist
+    assert abs(go.interior(Pc)[8]).max() > 0          # a heat flux has built up
+
+
 @pytest.mark.parametrize("nvar,ct", [(8, False), (10, True)])
 def test_minmod_with_two_ghost_zones(nvar, ct):
     """ng = 2 is enough for minmod (G-9): tiles, edge / fringe boxes and the EMHD slopes stay inside the padded array."""
