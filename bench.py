@@ -37,6 +37,15 @@ ALG_BYTES_PER_ZONE_STAGE_NEWTON = 8.0 * (10 + 10 + 10 + 10 + 3 + 10 + 1) + 4 * 4
 # dram__bytes_read.sum + dram__bytes_write.sum of the Newton kernel per zone, mean of the stage-1 and stage-2 launches of
 # one ncu --set full capture (profiles/r1g_ncu_full_stage_kernels.md: 4.82 GB and 6.16 GB per 256^3 launch)
 NCU_DRAM_BYTES_PER_ZONE_STAGE_NEWTON = 327.0
+NEWTON_KERNEL = "newton_stage_kernel<10,flat>"
+NCU_TRAFFIC_SOURCE = "profiles/r1g_ncu_full_stage_kernels.md"
+# Flux class (3 face-flux launches + boundary-face boxes + stage constant) per zone and stage.  Algorithmic bytes: SURVEY
+# 8(d) "Flux + stage constant, EMHD": P_E 10 (x 1.3-1.5 halo re-read) + P_n 10 in, C 10 + G 3 out -> 320-400 B; the
+# upper figure.  Algorithmic fp64 work: DADD + DMUL + DFMA thread instructions of the same four kernels in the round's
+# first ncu capture (profiles/r1a_ncu_full_stage_kernels_baseline.md), frozen like the Newton count.
+ALG_BYTES_PER_ZONE_STAGE_FLUX = 400.0
+ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX = 4370.0
+NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX = 1000.0
 FP64_INSTR_PER_CLK_PER_SM = 64.0                 # B200: 64 fp64 lanes per SM (guide: unit counts), 148 SMs
 N_SM = 148
 
@@ -99,12 +108,14 @@ class ClockSampler:
 def oracle_sample(n, steps, warmup):
     """The oracle, as it stands, on the config-3 generator at n^3; returns (zone-updates/s, s per step, cores)."""
     sys.path.insert(0, os.path.join(ROOT, "oracle"))
-    sys.path.insert(0, os.path.join(ROOT, "tests"))
     import oracle as og
-    from common import oracle_grid
     from paper_1702_01106_b200 import workloads
     gk, P = workloads.config3(n=n)
-    go = oracle_grid(gk)
+    go = og.Grid(gk["n1"], gk["n2"], gk["n3"], ng=gk.get("ng", 3), dim=gk["dim"], xstart=gk.get("xstart", (0, 0, 0)),
+                 xend=gk.get("xend", (1, 1, 1)), bc=gk.get("bc", og.BC_PERIODIC), nvar=gk["nvar"], recon=gk["recon"],
+                 gam=gk.get("gam", 4.0 / 3.0), phi=gk.get("phi", 1.0), psi=gk.get("psi", 1.0), tau=gk.get("tau", 1.0),
+                 fd_eps=gk.get("fd_eps", 4e-8), eps_bt=gk.get("eps_bt", 1e-4), atol=gk.get("atol", 0.0),
+                 rtol=gk.get("rtol", 1e-14), kmax=gk.get("kmax", 8), lsmax=gk.get("lsmax", 5), cfl=gk.get("cfl", 0.5))
     dt = go.choose_dt(P)
     for _ in range(warmup):
         go.timestep(P, dt)
@@ -210,11 +221,17 @@ def run_ours(args):
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the library has no CPU fallback")
+    if args.backend == "gloo":
+        local = local % torch.cuda.device_count()      # ranks may share a device (host-staged exchange; 1-GPU boxes)
     torch.cuda.set_device(local)
     if world > 1:
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if args.backend == "nccl":
+            os.environ.setdefault("NCCL_DEBUG", "WARN")
+            dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        else:
+            dist.init_process_group("gloo")
     n = args.n
-    gk, P0 = workloads.config3(n=n, ranks=world, rank=rank)
+    gk, P0 = workloads.config3(n=n, dim=args.dim, ranks=world, rank=rank)
     gk["flux_ct"] = bool(args.flux_ct)
     gk["reduced"] = bool(args.reduced)
     slab = gdist.SlabGrid(gk, world, rank, device=local)
@@ -273,30 +290,52 @@ def run_ours(args):
     stages = 2 * args.steps
     nk_ms, nk_n = timing["newton"]
     newton_ms = nk_ms / max(nk_n, 1)
+    flux_ms = timing["flux"][0] / stages                                       # all flux-class launches of one stage
     alu_peak = N_SM * FP64_INSTR_PER_CLK_PER_SM * sm_max * 1e6 / 1e12          # T fp64 thread-instr/s
-    alu_ach = ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON * zones / (newton_ms * 1e-3) / 1e12
+    # measured on this device, now: 8 independent DFMA chains per thread, 8 x 256 threads per SM (grim_fp64_probe)
+    probe = max(g.fp64_probe(True, 1 << 15) for _ in range(3)) / 1e12
+    headline = (not args.reduced) and (not args.flux_ct) and args.dim == 3
+    mean_it = None if st is None else [sum(i * st.iters_hist[s][i] for i in range(16)) / max(zones, 1) for s in range(2)]
+    # the frozen count is for 2 Newton iterations per zone and stage; other iteration counts scale it (set-up included:
+    # a slight overstatement of the work for > 2 iterations, an understatement for < 2)
+    it_scale = 1.0 if mean_it is None else 0.5 * (mean_it[0] + mean_it[1]) / 2.0
+    alu_ach = ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON * it_scale * zones / (newton_ms * 1e-3) / 1e12
     hbm_ach = ALG_BYTES_PER_ZONE_STAGE_NEWTON * zones / (newton_ms * 1e-3) / 1e9
+    flux_alu = ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX * zones / (flux_ms * 1e-3) / 1e12
+    flux_hbm = ALG_BYTES_PER_ZONE_STAGE_FLUX * zones / (flux_ms * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": zones * world * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "config3-emhd-mp5-llf-minkowski-%d^3%s" % (n, ("-fluxct" if args.flux_ct else "") + ("-reduced7" if args.reduced else "")),
+        "config": {"workload": "config3-emhd-mp5-llf-minkowski-%d^%d%s" % (n, args.dim, ("-fluxct" if args.flux_ct else "") + ("-reduced7" if args.reduced else "")),
                    "zones_per_gpu": zones,
                    "update": "one zone advanced one grim_timestep = 2 stages x (ghosts, MP5+LLF fluxes, stage "
                              "constants, fused Newton solve)", "dt": "fixed: CFL 0.5 on the initial data",
                    "l2": "inputs (%.2f GB per field) larger than L2" % (pbytes / 1e9),
-                   "parallelism": "slab%d" % world},
+                   "parallelism": "slab%d" % world, "backend": args.backend if world > 1 else None},
         "clocks": clocks,
         "e2e": {"value": zones * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": pbytes,
                 "d2h_bytes_per_step": pbytes},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "alu", "kernel": "newton_stage_kernel<10,flat>", "achieved": alu_ach, "peak": alu_peak,
-                     "unit": "T fp64 instr/s", "frac": alu_ach / alu_peak,
-                     "traffic": NCU_DRAM_BYTES_PER_ZONE_STAGE_NEWTON * zones,
-                     "peak_source": "148 SM x 64 fp64 lanes x %s sm_max_mhz %.0f" % (which, sm_max),
-                     "launch_ms": newton_ms, "launches": int(nk_n)},
-        "roofline_hbm": {"bound": "hbm", "kernel": "newton_stage_kernel<10,flat>", "achieved": hbm_ach,
-                         "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_ach / hbm_gbs, "peak_source": which},
+        "roofline": None if not headline else {
+            "bound": "alu", "kernel": NEWTON_KERNEL, "achieved": alu_ach, "peak": alu_peak,
+            "unit": "T fp64 instr/s", "frac": alu_ach / alu_peak,
+            "traffic": NCU_DRAM_BYTES_PER_ZONE_STAGE_NEWTON * zones, "traffic_source": NCU_TRAFFIC_SOURCE,
+            "peak_source": "148 SM x 64 fp64 lanes x %s sm_max_mhz %.0f" % (which, sm_max),
+            "peak_measured": probe, "peak_measured_source": "grim_fp64_probe (DFMA, 8 chains/thread), this run",
+            "frac_of_measured": alu_ach / probe,
+            "alg_fp64_instr_per_zone_stage": ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON * it_scale,
+            "mean_newton_iterations": mean_it, "launch_ms": newton_ms, "launches": int(nk_n)},
+        "roofline_hbm": None if not headline else {
+            "bound": "hbm", "kernel": NEWTON_KERNEL, "achieved": hbm_ach,
+            "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_ach / hbm_gbs, "peak_source": which},
+        "roofline_flux": None if not headline else {
+            "bound": "alu", "kernel": "face_flux_kernel x3 + stage_const (all flux-class launches of one stage)",
+            "achieved": flux_alu, "peak": alu_peak, "unit": "T fp64 instr/s", "frac": flux_alu / alu_peak,
+            "hbm_achieved_gbs": flux_hbm, "hbm_frac": flux_hbm / hbm_gbs,
+            "traffic": NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX * zones, "traffic_source": NCU_TRAFFIC_SOURCE,
+            "alg_fp64_instr_per_zone_stage": ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX,
+            "alg_bytes_per_zone_stage": ALG_BYTES_PER_ZONE_STAGE_FLUX, "stage_ms": flux_ms},
         "kernel_ms_per_step": {k: v[0] / args.steps for k, v in timing.items()},
         "newton_zone_iterations_per_s": (None if st is None else
                                          sum(i * (st.iters_hist[0][i] + st.iters_hist[1][i]) for i in range(16))
@@ -335,8 +374,26 @@ def main():
     ap.add_argument("--reduced", action="store_true",
                     help="the paper's reduced solve (B explicit, 7 x 7 Jacobian) instead of BASELINE's 10 unknowns")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads (config 2, Kerr step)")
+    ap.add_argument("--dim", type=int, default=3, choices=[2, 3], help="2: the same generator on an n x n grid (X^2 slabs)")
+    ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],
+                    help="N > 1: nccl = one GPU per rank, device-to-device ghost planes; gloo = host-staged planes, ranks "
+                         "may share a device (how a 1-GPU box exercises the N > 1 path)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # a plain `python bench.py --gpus N`: start one rank per GPU ourselves with the environment torchrun would set
+        # (torchrun's own argument parser rejects script options it can read as abbreviations of its own, e.g. --n)
+        import socket
+        sk = socket.socket()
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+        sk.close()
+        procs = []
+        for r in range(args.gpus):
+            env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(args.gpus), LOCAL_WORLD_SIZE=str(args.gpus),
+                       MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+            procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=env))
+        raise SystemExit(max(abs(p.wait()) for p in procs))
     if args.impl == "reference":
         run_reference(args)
     else:

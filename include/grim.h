@@ -155,7 +155,11 @@ int grim_newton_solve(grim_ctx *c, const double *P_n, const double *P_E, const d
 
 /* Standalone primitive recovery (O-10; BASELINE config 2): for each of nz zones solves
  * R(P) = (U(P) - U*)/||U*||_2 = 0 by the same Newton iteration, tol = rtol.
- *   U_target : N*nz flat   geom : NULL (Minkowski) -- curved-space flat inversion is not implemented (GRIM_EINVAL)
+ *   U_target : N*nz flat
+ *   geom : NULL (Minkowski), or the geometry of each zone, device double[15*nz], component-major [c*nz + z]:
+ *          c = 0..9 g_mu_nu in the order 00 01 02 03 11 12 13 22 23 33, c = 10..12 g^{t1} g^{t2} g^{t3},
+ *          c = 13 sqrt(-g), c = 14 the lapse alpha = 1/sqrt(-g^{tt}) (L248; C-9: beta^i/alpha = alpha g^{ti});
+ *          tau_R is the descriptor's constant tau
  *   P_inout : N*nz, guess -> result   iters, status : nz int32, out   resnorm : nz, out
  * Zones are solved to a terminal status; the active set is compacted between iteration sweeps. */
 int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_target, const double *geom, double *P_inout,

@@ -292,8 +292,9 @@ def llf(Fm, Fp, Um, Up, c):
     return F
 
 
-def invert(m, s, Ustar, Pguess, tau=1.0):
-    """Flat SoA [v][z] standalone inversion (O-10), Minkowski.  Returns P, iters, status, resnorm, backtracks."""
+def invert(m, s, Ustar, Pguess, tau=1.0, geoms=None):
+    """Flat SoA [v][z] standalone inversion (O-10); geoms: None (Minkowski) or one Geom per zone.
+    Returns P, iters, status, resnorm, backtracks."""
     Ustar = np.ascontiguousarray(Ustar, dtype=np.float64)
     P = np.array(Pguess, dtype=np.float64, order="C")
     nz = P.shape[1]
@@ -301,7 +302,11 @@ def invert(m, s, Ustar, Pguess, tau=1.0):
     status = np.zeros(nz, dtype=np.int32)
     resnorm = np.zeros(nz)
     bt = C.c_int64(0)
-    lib().og_invert(C.byref(m), C.byref(s), tau, nz, _d(Ustar), None, _d(P), _i(iters), _i(status),
+    garr = None
+    if geoms is not None:
+        assert len(geoms) == nz
+        garr = (Geom * nz)(*geoms)
+    lib().og_invert(C.byref(m), C.byref(s), tau, nz, _d(Ustar), garr, _d(P), _i(iters), _i(status),
                     _d(resnorm), C.byref(bt))
     return P, iters, status, resnorm, bt.value
 

@@ -245,10 +245,13 @@ class Grid:
                                               _ptr(P_out, t.float64), _ptr(resnorm, t.float64),
                                               _ptr(status, t.int32), _ptr(iters, t.int32)), "grim_newton_solve")
 
-    def invert_primitives(self, U_target, P_inout, iters, status, resnorm):
+    def invert_primitives(self, U_target, P_inout, iters, status, resnorm, geom=None):
+        """geom: None (Minkowski) or a [15, nz] CUDA tensor of per-zone geometry (layout: include/grim.h)."""
         t = self.torch
         nz = P_inout.shape[1]
-        self._check(self._L.grim_invert_primitives(self.h, nz, _ptr(U_target, t.float64), None,
+        if geom is not None and tuple(geom.shape) != (15, nz):
+            raise GrimError("invert_primitives: geom must have shape (15, %d)" % nz)
+        self._check(self._L.grim_invert_primitives(self.h, nz, _ptr(U_target, t.float64), _ptr(geom, t.float64),
                                                    _ptr(P_inout, t.float64), _ptr(iters, t.int32),
                                                    _ptr(status, t.int32), _ptr(resnorm, t.float64)),
                     "grim_invert_primitives")

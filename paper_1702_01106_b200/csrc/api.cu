@@ -404,7 +404,6 @@ extern "C" int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, 
 extern "C" int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_target, const double *geom,
                                       double *P_inout, int32_t *iters, int32_t *status, double *resnorm) {
   if (!c) return GRIM_EINVAL;
-  if (geom) return fail(c, GRIM_EINVAL, "curved-space flat inversion is not implemented; pass geom = NULL");
   if (nz < 0 || (nz > 0 && (!U_target || !P_inout || !iters || !status || !resnorm)))
     return fail(c, GRIM_EINVAL, "grim_invert_primitives: bad argument");
   if (nz == 0) return GRIM_OK;
@@ -424,7 +423,7 @@ extern "C" int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_t
   while (nlist > 0) {
     const int sweep = first ? GRIM_SWEEP_FIRST : GRIM_SWEEP_REST;
     CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
-    c->launches += timed(c, GRIM_K_INVERT, [&] { return launch_invert(c->gv, nz, nlist, c->list[cur], U_target, P_inout, iters, status, resnorm, sweep,
+    c->launches += timed(c, GRIM_K_INVERT, [&] { return launch_invert(c->gv, nz, nlist, c->list[cur], U_target, geom, P_inout, iters, status, resnorm, sweep,
                                  first, c->list[cur ^ 1], c->cnt, c->stream); });
     int rc = check_launch(c, "invert kernel");
     if (rc) return rc;

@@ -91,7 +91,7 @@ int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, 
                         const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
                         int32_t *iters, Counters *cnt, cudaStream_t s);
 int launch_invert(const GridView &gv, long long nz, long long nlist, const long long *list, const double *Ustar,
-                  double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters, int first,
+                  const double *geom, double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters, int first,
                   long long *next_list, Counters *cnt, cudaStream_t s);
 int launch_prim_to_conserved(const GridView &gv, long long nz, const double *P, double *U, cudaStream_t s);
 int launch_fluxes(const GridView &gv, const double *PE, const double *Pn, double dt_stage, double *C, double *G,

@@ -240,28 +240,51 @@ template <int N, class G>
 __global__ void stats_kernel(GridView gv, const double *__restrict__ Pn, double dt_stage,
                              const double *__restrict__ resnorm, const int32_t *__restrict__ status,
                              const int32_t *__restrict__ iters, StatsDev *out) {
+  // per-block histogram in shared memory, one global atomic per non-empty bin and block (the per-thread global
+  // atomics of the first version serialised 16.8 M updates on a handful of addresses: 18.6 ms at 256^3)
+  __shared__ unsigned int s_hist[16];
+  __shared__ unsigned int s_unconv;
+  __shared__ unsigned long long s_max;
+  if (threadIdx.x < 16) s_hist[threadIdx.x] = 0;
+  if (threadIdx.x == 16) s_unconv = 0;
+  if (threadIdx.x == 17) s_max = 0;
+  __syncthreads();
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= gv.nint) return;
-  int i, j, k;
-  zone_coords(gv, t, i, j, k);
-  const long long z = zone_index(gv, i, j, k);
-  int it = iters[z];
-  it = it > 15 ? 15 : it;
-  atomicAdd(&out->hist[it], 1ULL);
-  if (!(status[z] & ST_CONVERGED)) atomicAdd(&out->unconverged, 1ULL);
-  G g;
-  double tau = gv.tau_const;
-  if constexpr (!G::flat) load_geom<0>(gv.geomC, gv.n2d, (long long)j * gv.sz[0] + i, g, tau);
-  double P[N], U[N];
+  double rel = 0.0;
+  int unconv = 0;
+  if (t < gv.nint) {
+    int i, j, k;
+    zone_coords(gv, t, i, j, k);
+    const long long z = zone_index(gv, i, j, k);
+    int it = iters[z];
+    it = it > 15 ? 15 : it;
+    atomicAdd(&s_hist[it], 1u);
+    unconv = (status[z] & ST_CONVERGED) ? 0 : 1;
+    G g;
+    double tau = gv.tau_const;
+    if constexpr (!G::flat) load_geom<0>(gv.geomC, gv.n2d, (long long)j * gv.sz[0] + i, g, tau);
+    double P[N], U[N];
 #pragma unroll
-  for (int v = 0; v < N; v++) P[v] = Pn[v * gv.zg + z];
-  Pieces pc;
-  ExactArith ar;
-  full_state<N>(ar, gv.m, g, tau, P, pc.th, pc.v, pc.b, pc.h);
-  flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
-  const double sc = sqrt(norm2sq<N>(U)) / dt_stage;
-  const double rel = resnorm[z] / sc;
-  if (rel > 0.0) atomicMax(&out->max_rel, (unsigned long long)__double_as_longlong(rel));
+    for (int v = 0; v < N; v++) P[v] = Pn[v * gv.zg + z];
+    Pieces pc;
+    ExactArith ar;
+    full_state<N>(ar, gv.m, g, tau, P, pc.th, pc.v, pc.b, pc.h);
+    flux_vector<N>(g, 0, P, pc.th, pc.v, pc.b, pc.h, U);
+    const double sc = sqrt(norm2sq<N>(U)) / dt_stage;
+    rel = resnorm[z] / sc;
+    if (!(rel > 0.0)) rel = 0.0;
+  }
+  const unsigned nun = __reduce_add_sync(0xffffffffu, (unsigned)unconv);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) rel = fmax(rel, __shfl_xor_sync(0xffffffffu, rel, o));
+  if ((threadIdx.x & 31) == 0) {
+    if (nun) atomicAdd(&s_unconv, nun);
+    if (rel > 0.0) atomicMax(&s_max, (unsigned long long)__double_as_longlong(rel));
+  }
+  __syncthreads();
+  if (threadIdx.x < 16 && s_hist[threadIdx.x]) atomicAdd(&out->hist[threadIdx.x], (unsigned long long)s_hist[threadIdx.x]);
+  if (threadIdx.x == 16 && s_unconv) atomicAdd(&out->unconverged, (unsigned long long)s_unconv);
+  if (threadIdx.x == 17 && s_max) atomicMax(&out->max_rel, s_max);
 }
 
 int launch_stats(const GridView &gv, const double *Pn, double dt_stage, const double *resnorm,

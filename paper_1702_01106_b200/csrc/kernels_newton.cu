@@ -162,15 +162,26 @@ struct InvertArgs {
   double *resnorm;
   int max_iters, first;
   long long *next_list;
+  const double *geom;  // per-zone geometry, INV_GEOM_NCOMP x nz (include/grim.h), or null: Minkowski
 };
 
 // One zone of the standalone inversion under arithmetic policy A; same protocol as stage_zone.
-template <int N, class A>
+template <int N, class G, class A>
 __device__ __forceinline__ int invert_zone(A &ar, const GridView &gv, const InvertArgs &a, long long z, double *sj) {
-  InvertProblem<N, NB> prob;
+  InvertProblem<N, G, NB> prob;
   prob.m = gv.m;
   prob.Us = sj + N * N * NB;
   prob.tau_ = gv.tau_const;
+  if constexpr (!G::flat) {
+    // g_mu_nu (sym4 order), g^{t i}, sqrt(-g), alpha of this zone; beta^i/alpha = alpha g^{t i} (C-9)
+#pragma unroll
+    for (int c = 0; c < 10; c++) prob.g.g[c] = a.geom[c * a.nz + z];
+    prob.g.sg = a.geom[13 * a.nz + z];
+    prob.g.alpha = a.geom[14 * a.nz + z];
+#pragma unroll
+    for (int i = 0; i < 3; i++) prob.g.bfac[i] = prob.g.alpha * a.geom[(10 + i) * a.nz + z];
+    prob.g.gcon00 = prob.g.gcon0d = prob.g.gcondd = 0.0;
+  }
   double P[N];
 #pragma unroll
   for (int v = 0; v < N; v++) {
@@ -192,13 +203,13 @@ __device__ __forceinline__ int invert_zone(A &ar, const GridView &gv, const Inve
   return (nbt << 1) | ((st & ST_TERMINAL) ? 0 : 1);
 }
 
-template <int N>
+template <int N, class G>
 __device__ __noinline__ int invert_zone_replay(const GridView &gv, const InvertArgs &a, long long z, double *sj) {
   ExactArith ar;
-  return invert_zone<N>(ar, gv, a, z, sj);
+  return invert_zone<N, G>(ar, gv, a, z, sj);
 }
 
-template <int N>
+template <int N, class G>
 __global__ void __launch_bounds__(NB, N == 8 ? GRIM_N8_MINB : 256 / NB)
 invert_kernel(const __grid_constant__ GridView gv, const __grid_constant__ InvertArgs a, Counters *cnt) {
   extern __shared__ double smem[];
@@ -208,8 +219,8 @@ invert_kernel(const __grid_constant__ GridView gv, const __grid_constant__ Inver
   if (t < a.nlist) {
     z = a.first ? t : a.list[t];
     SpecArith ar;
-    res = invert_zone<N>(ar, gv, a, z, smem + threadIdx.x);
-    if (res < 0) res = invert_zone_replay<N>(gv, a, z, smem + threadIdx.x);
+    res = invert_zone<N, G>(ar, gv, a, z, smem + threadIdx.x);
+    if (res < 0) res = invert_zone_replay<N, G>(gv, a, z, smem + threadIdx.x);
   }
   const int active_after = res & 1;
   // warp-aggregated append to the next active list
@@ -223,25 +234,28 @@ invert_kernel(const __grid_constant__ GridView gv, const __grid_constant__ Inver
   if (lane == 0 && b) atomicAdd(&cnt->backtracks, b);
 }
 
-template <int N>
+template <int N, class G>
 static int launch_invert_t(const GridView &gv, long long nz, long long nlist, const long long *list,
-                           const double *Ustar, double *P, int32_t *iters, int32_t *status, double *resnorm,
-                           int max_iters, int first, long long *next_list, Counters *cnt, cudaStream_t s) {
+                           const double *Ustar, const double *geom, double *P, int32_t *iters, int32_t *status,
+                           double *resnorm, int max_iters, int first, long long *next_list, Counters *cnt,
+                           cudaStream_t s) {
   const size_t smem = (size_t)(N * N + N) * NB * sizeof(double);  // Jacobian + C (or U*) per thread
-  cudaFuncSetAttribute(invert_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  cudaFuncSetAttribute(invert_kernel<N, G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
   const long long blocks = (nlist + NB - 1) / NB;
   if (blocks == 0) return 0;
-  const InvertArgs a{nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list};
-  invert_kernel<N><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
+  const InvertArgs a{nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list, geom};
+  invert_kernel<N, G><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
   return 1;
 }
 
 int launch_invert(const GridView &gv, long long nz, long long nlist, const long long *list, const double *Ustar,
-                  double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters, int first,
-                  long long *next_list, Counters *cnt, cudaStream_t s) {
-  if (gv.nvar == 10)
-    return launch_invert_t<10>(gv, nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list, cnt, s);
-  return launch_invert_t<8>(gv, nz, nlist, list, Ustar, P, iters, status, resnorm, max_iters, first, next_list, cnt, s);
+                  const double *geom, double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters,
+                  int first, long long *next_list, Counters *cnt, cudaStream_t s) {
+#define GRIM_INV(NV, GG) \
+  launch_invert_t<NV, GG>(gv, nz, nlist, list, Ustar, geom, P, iters, status, resnorm, max_iters, first, next_list, cnt, s)
+  if (gv.nvar == 10) return geom ? GRIM_INV(10, GeomGen) : GRIM_INV(10, GeomFlat);
+  return geom ? GRIM_INV(8, GeomGen) : GRIM_INV(8, GeomFlat);
+#undef GRIM_INV
 }
 
 // U(P) on flat arrays, Minkowski (workload construction on the device)

@@ -102,16 +102,16 @@ struct StageProblem {
   }
 };
 
-template <int N, int CS>
+template <int N, class G, int CS>
 struct InvertProblem {
   ModelParams m;
-  GeomFlat g;
+  G g;
   double tau_;
   const double *Us;  // U*[v] at Us[v * CS] (shared memory)
   double iscale;
 
   __device__ __forceinline__ const ModelParams &model() const { return m; }
-  __device__ __forceinline__ const GeomFlat &geom() const { return g; }
+  __device__ __forceinline__ const G &geom() const { return g; }
   __device__ __forceinline__ double tau() const { return tau_; }
 
   template <class A>

@@ -1,4 +1,5 @@
-"""Slab decomposition of the grid along X^3 over torch.distributed ranks (one process per GPU).
+"""Slab decomposition of the grid along its slowest active direction -- X^3 of a 3-D grid, X^2 of a 2-D grid (SURVEY
+8(e)) -- over torch.distributed ranks (one process per GPU).
 
 The Newton solve, Jacobian, LU and line search are independent per zone; the only coupling between
 ranks is the stencil of the flux / explicit-gradient step, ng zones deep, so each stage needs ONE exchange of the
@@ -15,21 +16,22 @@ import torch
 import torch.distributed as dist
 
 
-def exchange_x3(P, ng, world, rank, periodic=True, group=None):
-    """Fills the X^3 ghost planes of the local padded array P[nvar, n3+2ng, s2, s1] from the neighbouring ranks'
-    interior planes (full padded X^1-X^2 planes, so edge and corner ghosts come along).  Rank r's lower neighbour is
-    r-1, upper r+1, wrapping if periodic; a missing neighbour leaves those ghosts untouched."""
+def exchange_slab(P, ng, world, rank, periodic=True, group=None, axis=1):
+    """Fills the ghost planes along tensor dimension `axis` (1: X^3, 2: X^2) of the local padded array
+    P[nvar, s3, s2, s1] from the neighbouring ranks' interior planes (full padded planes of the other directions, so
+    edge and corner ghosts come along).  Rank r's lower neighbour is r-1, upper r+1, wrapping if periodic; a missing
+    neighbour leaves those ghosts untouched."""
+    n = P.shape[axis] - 2 * ng
+    pl = lambda a, b: P.narrow(axis, a, b - a)       # planes [a, b) along the slab direction (a view)  # noqa: E731
     if world == 1:
         if periodic:
-            n3 = P.shape[1] - 2 * ng
-            P[:, :ng] = P[:, n3:n3 + ng]
-            P[:, ng + n3:] = P[:, ng:2 * ng]
+            pl(0, ng).copy_(pl(n, n + ng))
+            pl(ng + n, n + 2 * ng).copy_(pl(ng, 2 * ng))
         return
-    n3 = P.shape[1] - 2 * ng
     lo = rank - 1 if rank > 0 else (world - 1 if periodic else None)
     hi = rank + 1 if rank < world - 1 else (0 if periodic else None)
-    send_lo = P[:, ng:2 * ng].contiguous()             # my lowest interior planes -> lower neighbour's upper ghosts
-    send_hi = P[:, n3:n3 + ng].contiguous()            # my highest interior planes -> upper neighbour's lower ghosts
+    send_lo = pl(ng, 2 * ng).contiguous()            # my lowest interior planes -> lower neighbour's upper ghosts
+    send_hi = pl(n, n + ng).contiguous()             # my highest interior planes -> upper neighbour's lower ghosts
     if P.is_cuda and dist.get_backend(group) == "gloo":
         # gloo moves host memory only: stage the planes through the host (the NCCL path is device to device)
         send_lo, send_hi = send_lo.cpu(), send_hi.cpu()
@@ -50,30 +52,42 @@ def exchange_x3(P, ng, world, rank, periodic=True, group=None):
     for w in dist.batch_isend_irecv(ops):
         w.wait()
     if hi is not None:
-        P[:, ng + n3:] = recv_hi
+        pl(ng + n, n + 2 * ng).copy_(recv_hi)
     if lo is not None:
-        P[:, :ng] = recv_lo
+        pl(0, ng).copy_(recv_lo)
+
+
+def exchange_x3(P, ng, world, rank, periodic=True, group=None):
+    """exchange_slab along X^3."""
+    exchange_slab(P, ng, world, rank, periodic, group, axis=1)
 
 
 class SlabGrid:
-    """One rank's slab of an n1 x n2 x (world n3) grid.  world == 1 is the plain single-GPU grid."""
+    """One rank's slab of an n1 x n2 x (world n3) grid (3-D) or an n1 x (world n2) grid (2-D).  world == 1 is the plain
+    single-GPU grid."""
 
     def __init__(self, gk, world=1, rank=0, device=0):
         from . import binding as gb
         self.world, self.rank = world, rank
         k = dict(gk)
-        self.periodic3 = k.get("bc", gb.BC_PERIODIC) == gb.BC_PERIODIC if isinstance(k.get("bc", 0), int) else \
-            k["bc"][2][0] == gb.BC_PERIODIC
+        dim = k.get("dim", 3)
+        self.sdir = dim - 1                      # slab direction: the slowest active one (X^3, or X^2 of a 2-D grid)
+        self.axis = 3 - self.sdir                # its tensor dimension in P[nvar, s3, s2, s1]
         bc = k.get("bc", gb.BC_PERIODIC)
+        if isinstance(bc, int):
+            bc = [[bc, bc], [bc, bc], [bc, bc]]
+        bc = [list(b) for b in bc]
+        self.periodic3 = bc[self.sdir][0] == gb.BC_PERIODIC
         if world > 1:
-            if isinstance(bc, int):
-                bc = [[bc, bc], [bc, bc], [bc, bc]]
-            bc = [list(bc[0]), list(bc[1]), [gb.BC_NONE, gb.BC_NONE]]     # X^3 ghosts come from the neighbours
+            if dim < 2:
+                raise gb.GrimError("slab decomposition needs a 2-D or 3-D grid")
+            phys = bc[self.sdir]
+            bc[self.sdir] = [gb.BC_NONE, gb.BC_NONE]                       # these ghosts come from the neighbours
             if not self.periodic3:
                 if rank == 0:
-                    bc[2][0] = k["bc"][2][0]
+                    bc[self.sdir][0] = phys[0]
                 if rank == world - 1:
-                    bc[2][1] = k["bc"][2][1]
+                    bc[self.sdir][1] = phys[1]
         self.ng = k.get("ng", 3)
         self.grid = gb.Grid(k["n1"], k.get("n2", 1), k.get("n3", 1), ng=self.ng, dim=k.get("dim", 3),
                             xstart=k.get("xstart", (0, 0, 0)), xend=k.get("xend", (1, 1, 1)), bc=bc,
@@ -85,12 +99,10 @@ class SlabGrid:
                             lsmax=k.get("lsmax", 5), cfl=k.get("cfl", 0.5), metric=k.get("metric", 0),
                             metric_params=k.get("metric_params", ()), device=device,
                             flux_ct=k.get("flux_ct", False), reduced=k.get("reduced", False),
-                            riemann=k.get("riemann", 0))
+                            riemann=k.get("riemann", 0), closure=k.get("closure", 0))
         self.cfl = k.get("cfl", 0.5)
         g = self.grid
         if world > 1:
-            if g.ngd[2] == 0:
-                raise gb.GrimError("slab decomposition needs an active X^3 direction")
             t = torch
             self.Ph = g.zeros(g.nvar)
             self.rn = g.zeros()
@@ -100,7 +112,7 @@ class SlabGrid:
     def _ghosts(self, P):
         self.grid.fill_ghosts(P)
         if self.world > 1:
-            exchange_x3(P, self.ng, self.world, self.rank, self.periodic3)
+            exchange_slab(P, self.ng, self.world, self.rank, self.periodic3, axis=self.axis)
 
     def choose_dt(self, P):
         """dt = cfl / max over all ranks' zones of sum_d c^d/dX^d (C-15)."""

@@ -57,11 +57,14 @@ def config1(n=64, amp=1e-4):
 def config3(n=128, amp=1e-4, dim=3, recon=1, ranks=1, rank=0):
     """EMHD, 3-D Minkowski, n^3 periodic on [0,1]^3, four seeded random-phase linear modes, MP5, LLF, cfl 0.5.
     The headline run is the same generator at n = 256.  ranks > 1: rank's slab of the n x n x (ranks n) grid on
-    [0,1]^2 x [0,ranks] (the modes have period 1, so the stacked grid is periodic too)."""
+    [0,1]^2 x [0,ranks] (dim = 2: of the n x (ranks n) grid on [0,1] x [0,ranks]; the modes have period 1, so the
+    stacked grid is periodic too)."""
     t = mode_tables()["config3"]
     nn = (n, n, n if dim == 3 else 1)
-    grid = dict(n1=nn[0], n2=nn[1], n3=nn[2], ng=3, dim=dim, xstart=(0.0, 0.0, float(rank)),
-                xend=(1.0, 1.0, float(rank + 1)), nvar=10, recon=recon, limiter_theta=1.0, gam=t["gamma"],
+    xs, xe = [0.0, 0.0, 0.0], [1.0, 1.0, 1.0]
+    xs[dim - 1], xe[dim - 1] = float(rank), float(rank + 1)      # slabs along the slowest active direction
+    grid = dict(n1=nn[0], n2=nn[1], n3=nn[2], ng=3, dim=dim, xstart=tuple(xs),
+                xend=tuple(xe), nvar=10, recon=recon, limiter_theta=1.0, gam=t["gamma"],
                 phi=t["phi"], psi=t["psi"], tau=t["tau"], rtol=1e-14, kmax=8, lsmax=5, cfl=0.5)
     ngd = (3, 3, 3 if dim == 3 else 0)
     X = padded_centres(nn, ngd, grid["xstart"], grid["xend"])

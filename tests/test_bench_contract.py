@@ -55,3 +55,32 @@ def test_our_arm_json_line_small():
     assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["value"] > 0
     assert set(d["clocks"]) >= {"sm_mhz", "sm_max_mhz", "reasons"}
     assert d["vs_baseline"] is None and d["dtype"] == "f64" and d["data"] == "synthetic"
+
+
+def _run_two_ranks(backend):
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--backend", backend, "--n", "16",
+                        "--steps", "3", "--warmup", "3", "--no-extras", "--no-cpu-baseline"], capture_output=True,
+                       text=True, timeout=600)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [l for l in r.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                     # rank 0 alone prints
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["scaling"] == "weak" and d["config"]["parallelism"] == "slab2"
+    assert d["config"]["backend"] == backend and d["config"]["zones_per_gpu"] == 16 ** 3
+    assert abs(d["value"] - 2 * 16 ** 3 * 3 / (d["ms_per_step"] * 3e-3)) < 1e-6 * d["value"]
+    assert d["gpu_launches"] > 0 and d["e2e"]["value"] > 0
+
+
+@pytest.mark.gpu
+def test_bench_gpus2_plain_invocation_gloo_on_one_device():
+    """`python bench.py --gpus 2` with no torchrun environment starts its own two ranks; with --backend gloo they may
+    share the device (host-staged ghost planes), which is how a 1-GPU box runs the N > 1 code path end to end."""
+    _run_two_ranks("gloo")
+
+
+@pytest.mark.gpu
+def test_bench_gpus2_nccl():
+    import torch
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs: the NCCL path has not been run on hardware (DESIGN.md section 9)")
+    _run_two_ranks("nccl")

@@ -69,3 +69,43 @@ def test_exchange_single_rank_is_periodic_copy():
     exchange_x3(t, 2, 1, 0, True)
     assert np.array_equal(t.numpy()[:, :2, 2:6, 2:7], Q[:, :2, 2:6, 2:7])
     assert np.array_equal(t.numpy()[:, -2:, 2:6, 2:7], Q[:, -2:, 2:6, 2:7])
+
+
+def _worker2d(rank, world, port, bc2, n, ng, nvar, out):
+    """X^2 slabs of a 2-D grid: the stacked n1 x (world n2) grid with periodic X^1 and periodic /
+    outflow / polar-reflection X^2, ghosts filled the single-domain way by the oracle; each rank fills its own X^1
+    ghosts (as grim_fill_ghosts does, X^2 being BC_NONE towards a neighbour) and then exchanges."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    from paper_1702_01106_b200.distributed import exchange_slab
+    rng = np.random.default_rng(321)
+    gg = og.Grid(n[0], n[1] * world, 1, ng=ng, dim=2, nvar=nvar, bc=[[og.BC_PERIODIC] * 2, [bc2] * 2, [0, 0]])
+    Pg = rng.standard_normal(gg.shape)
+    gg.fill_ghosts(Pg)
+    j0 = ng + rank * n[1]
+    loc = np.full((nvar, 1, n[1] + 2 * ng, Pg.shape[3]), np.nan)
+    loc[:, :, ng:ng + n[1], ng:-ng] = Pg[:, :, j0:j0 + n[1], ng:-ng]          # interior only
+    periodic = bc2 == og.BC_PERIODIC
+    if not periodic:      # the physical boundary rows of the end ranks (the library fills them after X^1)
+        if rank == 0:
+            loc[:, :, :ng] = Pg[:, :, :ng]
+        if rank == world - 1:
+            loc[:, :, ng + n[1]:] = Pg[:, :, ng + n[1] * world:]
+    # X^1 ghosts of the interior rows: periodic copy (what fill_ghosts_kernel<0> does)
+    loc[:, :, ng:ng + n[1], :ng] = loc[:, :, ng:ng + n[1], n[0]:n[0] + ng]
+    loc[:, :, ng:ng + n[1], ng + n[0]:] = loc[:, :, ng:ng + n[1], ng:2 * ng]
+    t = torch.from_numpy(loc)
+    exchange_slab(t, ng, world, rank, periodic, axis=2)
+    expect = Pg[:, :, j0 - ng:j0 + n[1] + ng]
+    out[rank] = bool(np.array_equal(t.numpy(), expect))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("world,bc2", [(2, og.BC_PERIODIC), (3, og.BC_PERIODIC), (2, og.BC_OUTFLOW), (3, og.BC_REFLECT_POLAR)])
+def test_x2_slab_exchange_of_2d_grid_matches_single_domain_fill(world, bc2):
+    mgr = mp.Manager()
+    out = mgr.dict()
+    mp.spawn(_worker2d, args=(world, _free_port(), bc2, (6, 5), 3, 10, out), nprocs=world, join=True)
+    assert all(out[r] for r in range(world)), dict(out)

@@ -27,14 +27,14 @@ def _free_port():
     return p
 
 
-def _worker(rank, world, port, out):
+def _worker(rank, world, port, dim, out):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
     dist.init_process_group("gloo", rank=rank, world_size=world)
     torch.cuda.set_device(0)
     from paper_1702_01106_b200 import distributed as gdist
     from paper_1702_01106_b200 import workloads
-    gk, P0 = workloads.config3(n=N, ranks=world, rank=rank)
+    gk, P0 = workloads.config3(n=N, dim=dim, ranks=world, rank=rank)
     slab = gdist.SlabGrid(gk, world, rank, device=0)
     dP = torch.from_numpy(P0).cuda()
     dt = slab.choose_dt(dP)
@@ -45,15 +45,23 @@ def _worker(rank, world, port, out):
     dist.destroy_process_group()
 
 
-def test_two_ranks_equal_single_grid():
+@pytest.mark.parametrize("dim", [3, 2])
+def test_two_ranks_equal_single_grid(dim):
+    """dim = 3: slabs along X^3; dim = 2: slabs along X^2."""
     from paper_1702_01106_b200 import workloads
     world = 2
     mgr = mp.Manager()
     out = mgr.dict()
-    mp.spawn(_worker, args=(world, _free_port(), out), nprocs=world, join=True)
-    parts = [workloads.config3(n=N, ranks=world, rank=r) for r in range(world)]
-    gk = dict(parts[0][0], n3=world * N, xend=(1.0, 1.0, float(world)))
-    P = np.concatenate([parts[0][1][:, :NG + N], parts[1][1][:, NG:]], axis=1)
+    mp.spawn(_worker, args=(world, _free_port(), dim, out), nprocs=world, join=True)
+    parts = [workloads.config3(n=N, dim=dim, ranks=world, rank=r) for r in range(world)]
+    ax = 4 - dim                      # tensor dimension of the slab direction in P[nvar, s3, s2, s1]
+    if dim == 3:
+        gk = dict(parts[0][0], n3=world * N, xend=(1.0, 1.0, float(world)))
+    else:
+        gk = dict(parts[0][0], n2=world * N, xend=(1.0, float(world), 1.0))
+    lo = np.take(parts[0][1], range(NG + N), axis=ax)
+    hi = np.take(parts[1][1], range(NG, N + 2 * NG), axis=ax)
+    P = np.concatenate([lo, hi], axis=ax)
     g = cuda_grid(gk)
     dP = torch.from_numpy(np.ascontiguousarray(P)).cuda()
     dt, _ = g.timestep(dP.clone(), 0.0, want_dt=True)
@@ -62,6 +70,6 @@ def test_two_ranks_equal_single_grid():
     ref = dP.cpu().numpy()
     assert dt == out[0][0] == out[1][0]
     for r in range(world):
-        got = out[r][1][:, NG:NG + N, NG:-NG, NG:-NG]
-        exp = ref[:, NG + N * r:NG + N * (r + 1), NG:-NG, NG:-NG]
+        got = np.take(out[r][1], range(NG, NG + N), axis=ax)
+        exp = np.take(ref, range(NG + N * r, NG + N * (r + 1)), axis=ax)
         assert np.array_equal(got, exp)

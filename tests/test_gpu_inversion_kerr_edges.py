@@ -50,6 +50,46 @@ def test_invert_matches_oracle(nvar, nz):
         assert np.linalg.norm(Uz - U[:, z]) <= 1.0000001e-12 * np.linalg.norm(U[:, z]) * 1.5
 
 
+@pytest.mark.parametrize("nvar,nz", [(8, 6007), (10, 3001)])
+def test_invert_with_per_zone_kerr_geometry_matches_oracle(nvar, nz):
+    """grim_invert_primitives(geom != NULL) (SURVEY 8(b) geom_or_null; O-10): every zone carries the geometry of its
+    own point of the Kerr (a = 0.9375, MKS h = 0.3) spacetime, computed by the oracle and handed to both sides.
+    Statuses, iteration counts, residual norms and primitives bit-identical."""
+    import torch
+    from paper_1702_01106_b200 import workloads
+    rng = np.random.default_rng(31)
+    Ptrue, guess = workloads.config2(nz, seed=77, nvar=nvar)
+    X1 = rng.uniform(np.log(1.35), np.log(40.0), nz)
+    X2 = rng.uniform(0.02, 0.98, nz)
+    geoms = [og.kerr_mks(0.9375, 0.3, X1[z], X2[z]) for z in range(nz)]
+    m = og.model(nvar=nvar)
+    U = np.stack([og.prim_to_U(m, geoms[z], 1.0, Ptrue[:, z]) for z in range(nz)], axis=1)
+    s = og.solver(rtol=1e-12, kmax=30, lsmax=8)
+    Po, ito, sto, rno, _ = og.invert(m, s, U, guess, geoms=geoms)
+    garr = np.zeros((15, nz))
+    order = [(0, 0), (0, 1), (0, 2), (0, 3), (1, 1), (1, 2), (1, 3), (2, 2), (2, 3), (3, 3)]
+    for z, g in enumerate(geoms):
+        gcov, gcon, sg, al = og.geom_arrays(g)
+        garr[:10, z] = [gcov[a][b] for a, b in order]
+        garr[10:13, z] = gcon[0][1:4]
+        garr[13, z], garr[14, z] = sg, al
+    gc = cuda_grid(dict(n1=8, n2=8, n3=1, dim=2, nvar=nvar, rtol=1e-12, kmax=30, lsmax=8))
+    dP = to_dev(guess)
+    dit = torch.zeros(nz, dtype=torch.int32, device="cuda")
+    dst = torch.zeros_like(dit)
+    drn = torch.zeros(nz, dtype=torch.float64, device="cuda")
+    gc.invert_primitives(to_dev(U), dP, dit, dst, drn, geom=to_dev(garr))
+    assert np.array_equal(dst.cpu().numpy(), sto)
+    assert np.array_equal(dit.cpu().numpy(), ito)
+    assert np.array_equal(drn.cpu().numpy(), rno, equal_nan=True)
+    assert np.array_equal(dP.cpu().numpy(), Po, equal_nan=True)
+    assert ((sto & og.ST_CONVERGED) != 0).mean() > 0.2 and ito.max() > 6    # W up to 10 near the horizon: a hard set
+    # and the geometry mattered: the Minkowski solve of the same targets differs
+    dQ = to_dev(guess)
+    gc.invert_primitives(to_dev(U), dQ, dit, dst, drn)
+    assert not np.array_equal(dQ.cpu().numpy(), Po, equal_nan=True)
+
+
 def test_invert_host_entry_point_and_empty_input():
     import torch
     from paper_1702_01106_b200 import workloads

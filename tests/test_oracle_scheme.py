@@ -126,6 +126,36 @@ def test_round_trip_inversion():
     assert np.max(abs(Pr[:2, well] - P[:2, well]) / P[:2, well]) < 1e-9
 
 
+def test_round_trip_inversion_kerr_point_geometry():
+    """O-10 with geom_or_null given: every zone has its own Kerr (MKS, a = 0.9375) geometry.  P -> U(P) with
+    og_prim_to_U in that zone's geometry (itself pinned by the trace / Eckart-frame identities in Kerr) -> Newton from
+    a +-5 % guess -> P'.  A zone solved with another zone's geometry (or the Minkowski one) misses U by O(1)."""
+    rng = np.random.default_rng(9375)
+    nz = 600
+    P = _cfg2_like(rng, nz)
+    P[2:5] *= 0.2 / np.maximum(1.0, np.sqrt((P[2:5] ** 2).sum(0)))[None]      # moderate velocities: well conditioned
+    X1 = rng.uniform(np.log(1.5), np.log(40.0), nz)
+    X2 = rng.uniform(0.05, 0.95, nz)
+    geoms = [og.kerr_mks(0.9375, 0.3, X1[z], X2[z]) for z in range(nz)]
+    m = og.model(nvar=8)
+    U = np.stack([og.prim_to_U(m, geoms[z], 1.0, P[:, z]) for z in range(nz)], axis=1)
+    guess = P * (1 + 0.05 * rng.uniform(-1, 1, P.shape))
+    s = og.solver(rtol=1e-12, kmax=30, lsmax=8)
+    Pr, iters, status, resnorm, bt = og.invert(m, s, U, guess, geoms=geoms)
+    conv = (status & og.ST_CONVERGED) != 0
+    assert conv.mean() > 0.9
+    U2 = np.stack([og.prim_to_U(m, geoms[z], 1.0, Pr[:, z]) for z in range(nz)], axis=1)
+    rel = np.linalg.norm(U2 - U, axis=0) / np.linalg.norm(U, axis=0)
+    assert np.all(rel[conv] < 1.01e-12)
+    well = conv & ((P[5:8] ** 2).sum(0) / P[0] < 1) & (P[1] / P[0] > 1e-2) & (P[1] / P[0] < 1e2)
+    assert well.sum() > 30
+    assert np.max(abs(Pr[:2, well] - P[:2, well]) / P[:2, well]) < 1e-6      # conditioning x the 1e-12 residual
+    # negative control: the same targets solved in the wrong geometry (zone z+1's) do not reproduce P
+    Pw, _, stw, _, _ = og.invert(m, s, U, guess, geoms=geoms[1:] + geoms[:1])
+    bad = abs(Pw[:2, well] - P[:2, well]) / P[:2, well]
+    assert np.nanmedian(bad.max(axis=0)) > 1e-3
+
+
 def test_inversion_hydro_against_bisection():
     """P-11(iv): brute force.  B = 0 hydrodynamics reduces to a scalar equation for the pressure; solve it by
     bisection in numpy and compare with the oracle's Newton result."""
