@@ -266,6 +266,7 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   gv.flux_ct = d->flux_ct ? 1 : 0;
   gv.reduced = d->reduced_solve ? 1 : 0;
   gv.emf = c->emf;
+  gv.nsm = prop.multiProcessorCount;
   cudaMemsetAsync(c->G, 0, 3 * zg * 8, c->stream);
   cudaMemsetAsync(c->C, 0, N * zg * 8, c->stream);
   *out = c;

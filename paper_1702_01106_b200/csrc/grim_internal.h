@@ -37,6 +37,7 @@ struct GridView {
   int flux_ct;               // flux-CT averaging of the B-field fluxes
   int reduced;               // reduced solve: B^i explicit, Newton on the other N - 3 primitives
   double *emf;               // 3 * zg edge fields (flux_ct only)
+  int nsm;                   // multiprocessors of the device (persistent kernels)
 };
 
 // per-call device counters

@@ -29,9 +29,13 @@ template <int N, class G, bool RED, class A>
 __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const StageArgs &a, long long z, int i, int j,
                                           int st, double *sj) {
   constexpr int M = Unknowns<N, RED>::M;
-  StageProblem<N, G, NB> prob;
+  // EMHD full solve: the constants of the q / dP rows go to the unused words of the Jacobian's B rows
+  constexpr bool KSM = GRIM_KSM && N == 10 && use_structure<N, RED>();
+  static_assert(!KSM || K_COUNT <= 3 * (N - 1), "constants do not fit the free Jacobian words");
+  StageProblem<N, G, NB, KSM> prob;
   prob.m = gv.m;
   prob.Cs = sj + M * M * NB;
+  prob.Ks = sj;
   if constexpr (G::flat) {
     prob.tau_ = gv.tau_const;
   } else {
@@ -58,13 +62,14 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
         else P[B1 + d] = ar.div_z(b, prob.g.sqrtmg());
       }
     }
+    double Xq = 0.0, Xd = 0.0, divx = 0.0;
     if constexpr (N == 10) {
-      prob.Xq = a.Gx[0 * gv.zg + z];
-      prob.Xd = a.Gx[1 * gv.zg + z];
-      prob.divx = a.Gx[2 * gv.zg + z];
+      Xq = a.Gx[0 * gv.zg + z];
+      Xd = a.Gx[1 * gv.zg + z];
+      divx = a.Gx[2 * gv.zg + z];
     }
     full_state<N>(ar, prob.m, prob.g, prob.tau_, P, pc0.th, pc0.v, pc0.b, pc0.h);
-    prob.setup(ar, Pn_z, PE_z, a.dt_stage, pc0, !RED && a.PE == a.Pguess, !RED && a.Pn == a.Pguess);
+    prob.setup(ar, Pn_z, PE_z, a.dt_stage, pc0, !RED && a.PE == a.Pguess, !RED && a.Pn == a.Pguess, Xq, Xd, divx);
   }
   const double tol = gv.sp.atol + gv.sp.rtol * prob.scale;
   int it = a.fresh ? 0 : a.iters[z];

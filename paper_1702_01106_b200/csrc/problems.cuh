@@ -8,23 +8,49 @@
 
 namespace grim {
 
+// The P_n- / P_E-derived constants of the EMHD rows (O-8), frozen during the iteration.
+enum {
+  K_THN, K_UCOVN0, K_UCOVN1, K_UCOVN2, K_UCOVN3, K_UTN, K_QTN, K_DTN,           // P_n
+  K_BH0, K_BH1, K_BH2, K_BH3, K_THE, K_UTE, K_NRHOCHI, K_RHONU3, K_FQE, K_FDE,  // P_E
+  K_HQTE, K_HDTE, K_XQ, K_XD, K_DIVX, K_ITAU,
+  K_COUNT
+};
+
+// Where the constants live.  KSM = false: in registers.  KSM = true: in the thread's shared-memory words that the
+// structured solve leaves unused -- the off-diagonal entries of the Jacobian's B rows (newton.cuh: 27 words, never
+// written or read) -- which frees 2 K_COUNT registers for the finite-difference columns; constant i sits at
+// Ks[kslot(i) * CS].
+template <int N>
+__host__ __device__ constexpr int kslot(int i) {
+  const int r = B1 + i / (N - 1), c = i % (N - 1);
+  return r * N + (c < r ? c : c + 1);
+}
+#ifndef GRIM_KSM
+#define GRIM_KSM 1
+#endif
+
 // CS: stride (in doubles) of the per-thread shared-memory vector that holds the stage constant C
-template <int N, class G, int CS>
+template <int N, class G, int CS, bool KSM = false>
 struct StageProblem {
   ModelParams m;
   G g;
-  double tau_, idt, itau;
+  double tau_, idt;
   const double *Cs;  // C[v] at Cs[v * CS] (shared memory: read once per residual evaluation, 2N registers saved)
+  double *Ks;        // KSM: the thread's Jacobian base (shared memory)
   double scale;      // ||U(P_n)||_2 / dt' (C-2)
-  // EMHD only.  P_n-derived:
-  double Thn, ucovn[4], utn, qtn, dtn;
-  // P_E-derived coefficients, frozen during the iteration (O-8), and the spatial-gradient terms of the stage:
-  double bh[4], ThE, utE, nrhochi, rhonu3, fqE, fdE, hqtE, hdtE;
-  double Xq, Xd, divx;
+  double kreg[KSM ? 1 : K_COUNT];
 
   __device__ __forceinline__ const ModelParams &model() const { return m; }
   __device__ __forceinline__ const G &geom() const { return g; }
   __device__ __forceinline__ double tau() const { return tau_; }
+  __device__ __forceinline__ double K(int i) const {
+    if constexpr (KSM) return Ks[kslot<N>(i) * CS];
+    else return kreg[i];
+  }
+  __device__ __forceinline__ void setK(int i, double v) {
+    if constexpr (KSM) Ks[kslot<N>(i) * CS] = v;
+    else kreg[i] = v;
+  }
 
   // Everything that depends only on P_n and P_E (L438)
   template <class A>
@@ -32,9 +58,9 @@ struct StageProblem {
   // P_E, and in its first stage P_n is P_E too: the states of P_E / P_n are then pc0 itself (same inputs, same code,
   // same bits) and are not computed again.
   __device__ __forceinline__ void setup(A &ar, const double (&Pn)[N], const double (&PE)[N], double dt_stage,
-                                        const Pieces &pc0, bool pe_is_guess, bool pn_is_guess) {
+                                        const Pieces &pc0, bool pe_is_guess, bool pn_is_guess, double Xq, double Xd,
+                                        double divx) {
     idt = ar.rcp(dt_stage);
-    itau = ar.rcp(tau_);
     Pieces pn;
     if (pn_is_guess) pn = pc0;
     else full_state<N>(ar, m, g, tau_, Pn, pn.th, pn.v, pn.b, pn.h);
@@ -42,28 +68,33 @@ struct StageProblem {
     flux_vector<N>(g, 0, Pn, pn.th, pn.v, pn.b, pn.h, Un);
     scale = ar.sqrt_z(norm2sq<N>(Un)) * idt;
     if constexpr (N == 10) {
-      Thn = pn.th.Th;
+      setK(K_ITAU, ar.rcp(tau_));
+      setK(K_XQ, Xq);
+      setK(K_XD, Xd);
+      setK(K_DIVX, divx);
+      setK(K_THN, pn.th.Th);
 #pragma unroll
-      for (int i = 0; i < 4; i++) ucovn[i] = pn.v.ucov[i];
-      utn = pn.v.ucon[0];
-      qtn = Pn[QQ] * pn.th.fq;
-      dtn = Pn[DPP] * pn.th.fdp;
+      for (int i = 0; i < 4; i++) setK(K_UCOVN0 + i, pn.v.ucov[i]);
+      setK(K_UTN, pn.v.ucon[0]);
+      setK(K_QTN, Pn[QQ] * pn.th.fq);
+      setK(K_DTN, Pn[DPP] * pn.th.fdp);
       Pieces pe;
       if (pe_is_guess) pe = pc0;
       else full_state<N>(ar, m, g, tau_, PE, pe.th, pe.v, pe.b, pe.h);
 #pragma unroll
-      for (int i = 0; i < 4; i++) bh[i] = pe.h.con[i];
-      ThE = pe.th.Th;
-      utE = pe.v.ucon[0];
+      for (int i = 0; i < 4; i++) setK(K_BH0 + i, pe.h.con[i]);
+      setK(K_THE, pe.th.Th);
+      setK(K_UTE, pe.v.ucon[0]);
       double cs2 = sound_speed2(ar, m, PE[RHO], PE[UU]);
       double chi, nu;
       closure_coeffs(m, cs2, tau_, chi, nu);
-      nrhochi = -(PE[RHO] * chi);
-      rhonu3 = 3.0 * PE[RHO] * nu;
-      fqE = pe.th.fq;
-      fdE = pe.th.fdp;
-      hqtE = 0.5 * (PE[QQ] * fqE);
-      hdtE = 0.5 * (PE[DPP] * fdE);
+      setK(K_NRHOCHI, -(PE[RHO] * chi));
+      setK(K_RHONU3, 3.0 * PE[RHO] * nu);
+      const double fqE = pe.th.fq, fdE = pe.th.fdp;
+      setK(K_FQE, fqE);
+      setK(K_FDE, fdE);
+      setK(K_HQTE, 0.5 * (PE[QQ] * fqE));
+      setK(K_HDTE, 0.5 * (PE[DPP] * fdE));
     }
   }
 
@@ -74,23 +105,23 @@ struct StageProblem {
     for (int v = 0; v < N; v++) R[v] = U[v] * idt + Cs[v * CS];
     if constexpr (N == 10) {
       // time derivatives of derived quantities between the unknown state and P_n (C-3)
-      double dtTheta = (pc.th.Th - Thn) * idt;
+      double dtTheta = (pc.th.Th - K(K_THN)) * idt;
       double dtucov[4];
 #pragma unroll
-      for (int i = 0; i < 4; i++) dtucov[i] = (pc.v.ucov[i] - ucovn[i]) * idt;
-      double dtut = (pc.v.ucon[0] - utn) * idt;
-      double bdu = bh[0] * dtucov[0];
-      bdu = bdu + bh[1] * dtucov[1];
-      bdu = bdu + bh[2] * dtucov[2];
-      bdu = bdu + bh[3] * dtucov[3];
-      double Tq = bh[0] * dtTheta + ThE * (utE * bdu);
-      double Td = bh[0] * bdu;
-      double divu = dtut + divx;
-      double q0 = nrhochi * (Tq + Xq);                              // eq 37
-      double dP0 = rhonu3 * ((Td + Xd) - (1.0 / 3.0) * divu);        // eq 38 (G-5)
+      for (int i = 0; i < 4; i++) dtucov[i] = (pc.v.ucov[i] - K(K_UCOVN0 + i)) * idt;
+      double dtut = (pc.v.ucon[0] - K(K_UTN)) * idt;
+      double bdu = K(K_BH0) * dtucov[0];
+      bdu = bdu + K(K_BH1) * dtucov[1];
+      bdu = bdu + K(K_BH2) * dtucov[2];
+      bdu = bdu + K(K_BH3) * dtucov[3];
+      double Tq = K(K_BH0) * dtTheta + K(K_THE) * (K(K_UTE) * bdu);
+      double Td = K(K_BH0) * bdu;
+      double divu = dtut + K(K_DIVX);
+      double q0 = K(K_NRHOCHI) * (Tq + K(K_XQ));                              // eq 37
+      double dP0 = K(K_RHONU3) * ((Td + K(K_XD)) - (1.0 / 3.0) * divu);        // eq 38 (G-5)
       double qt = P[QQ] * pc.th.fq, dpt = P[DPP] * pc.th.fdp;
-      double Sq = -(0.5 * (qt + qtn) - fqE * q0) * itau + hqtE * divu;    // eq 39, eqs 15-16
-      double Sd = -(0.5 * (dpt + dtn) - fdE * dP0) * itau + hdtE * divu;  // eq 40
+      double Sq = -(0.5 * (qt + K(K_QTN)) - K(K_FQE) * q0) * K(K_ITAU) + K(K_HQTE) * divu;    // eq 39, eqs 15-16
+      double Sd = -(0.5 * (dpt + K(K_DTN)) - K(K_FDE) * dP0) * K(K_ITAU) + K(K_HDTE) * divu;  // eq 40
       if constexpr (G::flat) {
         R[QQ] = R[QQ] - Sq;
         R[DPP] = R[DPP] - Sd;
