@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <string>
@@ -46,9 +47,12 @@ struct grim_ctx {
   long long *list[2];          // inversion active lists
   long long list_cap;
   double *hostP;               // staging for the *_host entry points
+  cudaStream_t s_in, s_out;    // copy streams of the pipelined grim_timestep_host
+  std::vector<cudaEvent_t> ev_in, ev_done;
   double *invbuf;              // U, P, resnorm, iters, status of grim_invert_primitives_host
   long long invbuf_nz;
   int64_t launches;
+  int no_pipeline;             // GRIM_HOST_PIPELINE=0 in the environment: grim_timestep_host copies, steps, copies
   // optional per-kernel-class timing (grim_set_timing): event pairs recorded around the launches
   int timing;
   std::vector<KernelSpan> spans;
@@ -153,6 +157,10 @@ extern "C" void grim_free(grim_ctx *c) {
                   c->list[0], c->list[1], c->hostP, c->invbuf};
   for (void *p : ptrs)
     if (p) cudaFree(p);
+  for (auto e : c->ev_in) cudaEventDestroy(e);
+  for (auto e : c->ev_done) cudaEventDestroy(e);
+  if (c->s_in) cudaStreamDestroy(c->s_in);
+  if (c->s_out) cudaStreamDestroy(c->s_out);
   delete c;
 }
 
@@ -198,6 +206,11 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   c->stream = (cudaStream_t)d->stream;
   c->metric_set = 0;
   c->launches = 0;
+  c->s_in = c->s_out = nullptr;
+  {
+    const char *e = getenv("GRIM_HOST_PIPELINE");
+    c->no_pipeline = (e && e[0] == '0') ? 1 : 0;
+  }
   c->timing = 0;
   for (int k = 0; k < GRIM_NKCLASS; k++) { c->class_ms[k] = 0.0; c->class_n[k] = 0; }
   GridView &gv = c->gv;
@@ -584,6 +597,99 @@ extern "C" int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t
   return check_launch(c, "arith selftest");
 }
 
+// One time step with HOST buffers, pipelined over K slabs of X^3 planes: the host -> device copy of slab c + 1, the
+// kernels of slab c (stage 1) and c - 1 (stage 2) and the device -> host copy of slab c - 2 run at the same time on three
+// streams.  A slab's stage 1 needs P_n of the neighbouring slabs (stencil of the flux step, 3 + 1 planes), its stage 2
+// P_{n+1/2} of the neighbouring slabs; the X^3 boundary (periodic wrap or a physical boundary) couples the first and
+// the last slab, which therefore arrive first and finish last.  All kernels run on the context's stream in an order
+// that keeps every read ahead of the write that would overwrite it (stage 2 writes P_{n+1} over P_n in place); the
+// results are those of grim_timestep bit for bit.  Ghost zones of P_host are neither read nor written.
+#ifndef GRIM_HOST_SLABS
+#define GRIM_HOST_SLABS 16
+#endif
+static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
+  const GridView &gv = c->gv;
+  cudaStream_t s = c->stream;
+  const int K = GRIM_HOST_SLABS, ng = gv.ngd[2], n3 = gv.n[2];
+  const size_t plane = (size_t)gv.sz[0] * gv.sz[1], pitch = (size_t)gv.zg * 8;
+  if (!c->s_in) CU(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
+  if (!c->s_out) CU(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+  while ((int)c->ev_in.size() < K + 1) {
+    cudaEvent_t e;
+    CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    c->ev_in.push_back(e);
+    CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    c->ev_done.push_back(e);
+  }
+  int k0[GRIM_HOST_SLABS + 1];
+  for (int q = 0; q <= K; q++) k0[q] = (int)((long long)n3 * q / K / 4 * 4);  // multiples of the 4-plane flux tiles
+  k0[K] = n3;
+  double *d = c->hostP;
+  // the copy streams start after whatever the caller enqueued on the context's stream
+  CU(cudaEventRecord(c->ev_in[K], s));
+  CU(cudaStreamWaitEvent(c->s_in, c->ev_in[K], 0));
+  CU(cudaStreamWaitEvent(c->s_out, c->ev_in[K], 0));
+  auto h2d = [&](int q) {
+    const size_t off = (size_t)(ng + k0[q]) * plane;
+    cudaMemcpy2DAsync(d + off, pitch, P_host + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
+                      cudaMemcpyHostToDevice, c->s_in);
+    cudaEventRecord(c->ev_in[q], c->s_in);
+  };
+  h2d(K - 1);
+  for (int q = 0; q < K - 1; q++) h2d(q);
+  auto slab = [&](int q) {
+    GridView g = gv;
+    g.koff = k0[q];
+    g.n[2] = k0[q + 1] - k0[q];
+    g.nint = (long long)g.n[0] * g.n[1] * g.n[2];
+    return g;
+  };
+  auto ghosts01 = [&](double *P, int q) {  // X^1, X^2 ghosts of the slab's planes
+    c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(gv, c->d.bc, P, s, 3, ng + k0[q], k0[q + 1] - k0[q]); });
+  };
+  auto ghosts2 = [&](double *P) {
+    c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(gv, c->d.bc, P, s, 4); });
+  };
+  const double dt1 = 0.5 * dt;
+  auto stage1 = [&](int q) {
+    const GridView g = slab(q);
+    c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(g, d, d, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s); });
+    c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(g, d, d, c->C, c->G, d, 1, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s); });
+  };
+  auto stage2 = [&](int q) {
+    const GridView g = slab(q);
+    c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(g, c->Ph, d, dt, c->C, c->G, c->Fface, c->cface, nullptr, s); });
+    c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(g, d, c->Ph, c->C, c->G, c->Ph, 1, dt, 0, d, c->resnorm, c->status, c->iters, c->cnt, s); });
+    cudaEventRecord(c->ev_done[q], s);
+    cudaStreamWaitEvent(c->s_out, c->ev_done[q], 0);
+    const size_t off = (size_t)(ng + k0[q]) * plane;
+    cudaMemcpy2DAsync(P_host + off, pitch, d + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
+                      cudaMemcpyDeviceToHost, c->s_out);
+  };
+  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
+  CU(cudaStreamWaitEvent(s, c->ev_in[K - 1], 0));
+  CU(cudaStreamWaitEvent(s, c->ev_in[0], 0));
+  ghosts01(d, K - 1);
+  ghosts01(d, 0);
+  ghosts2(d);
+  for (int q = 0; q < K; q++) {
+    if (q + 1 <= K - 2) {
+      CU(cudaStreamWaitEvent(s, c->ev_in[q + 1], 0));
+      ghosts01(d, q + 1);
+    }
+    stage1(q);
+    ghosts01(c->Ph, q);
+    if (q >= 2) stage2(q - 1);
+  }
+  ghosts2(c->Ph);
+  stage2(K - 1);
+  stage2(0);
+  int rc = check_launch(c, "pipelined timestep");
+  CU(cudaStreamSynchronize(c->s_out));
+  CU(cudaStreamSynchronize(s));
+  return rc;
+}
+
 extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used) {
   int rc = need_metric(c);
   if (rc) return rc;
@@ -591,6 +697,18 @@ extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, d
   CU(cudaSetDevice(c->d.device));
   const size_t pbytes = (size_t)c->gv.nvar * c->gv.zg * 8;
   if (!c->hostP) CU(cudaMalloc((void **)&c->hostP, pbytes));
+  {
+    bool caller_ghosts = false;
+    for (int a = 0; a < 3; a++)
+      for (int sd = 0; sd < 2; sd++)
+        if (c->gv.ngd[a] > 0 && c->d.bc[a][sd] == GRIM_BC_NONE) caller_ghosts = true;
+    if (nsteps == 1 && dt > 0.0 && c->gv.dim == 3 && c->gv.n[2] >= 4 * GRIM_HOST_SLABS && !c->gv.flux_ct && !caller_ghosts &&
+        !c->no_pipeline) {
+      rc = timestep_host_pipelined(c, P_host, dt);
+      if (rc == GRIM_OK && dt_used) *dt_used = dt;
+      return rc;
+    }
+  }
   CU(cudaMemcpyAsync(c->hostP, P_host, pbytes, cudaMemcpyHostToDevice, c->stream));
   for (int s = 0; s < nsteps; s++) {
     rc = grim_timestep(c, c->hostP, dt, dt_used, nullptr);

@@ -37,7 +37,9 @@ struct GridView {
   int flux_ct;               // flux-CT averaging of the B-field fluxes
   int reduced;               // reduced solve: B^i explicit, Newton on the other N - 3 primitives
   double *emf;               // 3 * zg edge fields (flux_ct only)
-  int nsm;                   // multiprocessors of the device (persistent kernels)
+  int nsm;                   // multiprocessors of the device
+  int koff;                  // launches over a range of X^3 planes (pipelined host path): the interior zones are
+                             // those of planes [koff, koff + n[2]) of the grid; sz, zg, n2d keep the full extents
 };
 
 // per-call device counters
@@ -59,7 +61,7 @@ __host__ __device__ inline void zone_coords(const GridView &gv, long long t, int
   i = (int)(t % gv.n[0]) + gv.ngd[0];
   long long r = t / gv.n[0];
   j = (int)(r % gv.n[1]) + gv.ngd[1];
-  k = (int)(r / gv.n[1]) + gv.ngd[2];
+  k = (int)(r / gv.n[1]) + gv.ngd[2] + gv.koff;
 }
 __host__ __device__ inline long long zone_index(const GridView &gv, int i, int j, int k) {
   return ((long long)k * gv.sz[1] + j) * gv.sz[0] + i;
@@ -97,7 +99,10 @@ int launch_invert(const GridView &gv, long long nz, long long nlist, const long 
 int launch_prim_to_conserved(const GridView &gv, long long nz, const double *P, double *U, cudaStream_t s);
 int launch_fluxes(const GridView &gv, const double *PE, const double *Pn, double dt_stage, double *C, double *G,
                   double *Fface, double *cface, Counters *cnt, cudaStream_t s);
-int launch_fill_ghosts(const GridView &gv, const int32_t bc[3][2], double *P, cudaStream_t s);
+// dirs: bit a set = fill the ghosts of direction a; planes [klo, klo + kcnt) of the padded X^3 extent (kcnt < 0: all)
+// for the directions other than X^3
+int launch_fill_ghosts(const GridView &gv, const int32_t bc[3][2], double *P, cudaStream_t s, int dirs = 7,
+                       int klo = 0, int kcnt = -1);
 int launch_metric_kerr(const GridView &gv, double a, double h, int tau_mode, double *geomC, double *geomF0,
                        double *geomF1, double *geomF2, double *conn, cudaStream_t s);
 int launch_metric_flat(const GridView &gv, double *geomC, double *geomF0, double *geomF1, double *geomF2,

@@ -127,7 +127,7 @@ face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__
 
   // padded coordinates of the tile's first face, and of the first staged zone (LO zones below it along DIR)
   const int fi = gv.ngd[0] + (int)blockIdx.x * T::T0, fj = gv.ngd[1] + (int)blockIdx.y * T::T1,
-            fk = gv.ngd[2] + (int)blockIdx.z * T::T2;
+            fk = gv.ngd[2] + gv.koff + (int)blockIdx.z * T::T2;
   const int zi = fi - (DIR == 0 ? LO : 0), zj = fj - (DIR == 1 ? LO : 0), zk = fk - (DIR == 2 ? LO : 0);
   constexpr int ITER = (EZ + FB - 1) / FB;
 #pragma unroll
@@ -151,7 +151,7 @@ face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__
   const int i = fi + t0, j = fj + t1, k = fk + t2;
   // the tiles cover the n lower faces of the interior zones; the one upper boundary face per line goes to
   // face_edge_kernel, so that the tile grid divides the interior evenly
-  if (i >= gv.ngd[0] + gv.n[0] || j >= gv.ngd[1] + gv.n[1] || k >= gv.ngd[2] + gv.n[2]) return;
+  if (i >= gv.ngd[0] + gv.n[0] || j >= gv.ngd[1] + gv.n[1] || k >= gv.ngd[2] + gv.koff + gv.n[2]) return;
   const long long z = zone_index(gv, i, j, k);
   SpecArith ar;
   double F[N], c;
@@ -545,7 +545,7 @@ stage_const_tiled_kernel(const __grid_constant__ GridView gv, const double *__re
   using TF = TileFlux<N, T0, T1>;
   __shared__ double tile[TF::SIZE];
   const int i0 = gv.ngd[0] + (int)blockIdx.x * T0, j0 = gv.ngd[1] + (int)blockIdx.y * T1,
-            k = gv.ngd[2] + (int)blockIdx.z;
+            k = gv.ngd[2] + gv.koff + (int)blockIdx.z;
   const long long zg = gv.zg;
   // the zone's own primitives are requested first, so that they arrive while the tile is being staged
   const int t0 = (int)threadIdx.x % T0, t1 = (int)threadIdx.x / T0;
@@ -640,6 +640,7 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
     }
     edge.lo[a] = gv.ngd[a] + gv.n[a];
     edge.cnt[a] = 1;
+    edge.lo[2] += gv.koff;  // launches over a range of X^3 planes (flux-CT fringes are not offered there)
     box(edge);
     if (ext) {
       bool first = true;  // the first transverse direction takes the corners shared with the second

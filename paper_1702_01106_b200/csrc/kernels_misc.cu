@@ -183,12 +183,12 @@ int launch_metric_flat(const GridView &gv, double *geomC, double *geomF0, double
 // of the other directions, so that corners end up filled.
 // ---------------------------------------------------------------------------------------------------------
 template <int DIR>
-__global__ void fill_ghosts_kernel(GridView gv, int bc_lo, int bc_hi, double *__restrict__ P) {
+__global__ void fill_ghosts_kernel(GridView gv, int bc_lo, int bc_hi, double *__restrict__ P, int klo, int kcnt) {
   const int ng = gv.ngd[DIR], n = gv.n[DIR];
   // ghost layer index g in [0, 2 ng): lower side g < ng, upper side g >= ng
   const int e0 = (DIR == 0) ? 2 * ng : gv.sz[0];
   const int e1 = (DIR == 1) ? 2 * ng : gv.sz[1];
-  const int e2 = (DIR == 2) ? 2 * ng : gv.sz[2];
+  const int e2 = (DIR == 2) ? 2 * ng : kcnt;
   const long long per_var = (long long)e0 * e1 * e2;
   const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= per_var * gv.nvar) return;
@@ -200,6 +200,7 @@ __global__ void fill_ghosts_kernel(GridView gv, int bc_lo, int bc_hi, double *__
   c[1] = (int)(r % e1);
   c[2] = (int)(r / e1);
   const int gl = c[DIR];
+  if (DIR != 2) c[2] += klo;
   const int side = (gl >= ng) ? 1 : 0;
   const int gz = side ? gl - ng : gl;
   const int bc = side ? bc_hi : bc_lo;
@@ -217,17 +218,23 @@ __global__ void fill_ghosts_kernel(GridView gv, int bc_lo, int bc_hi, double *__
   P[v * gv.zg + zone_index(gv, cd[0], cd[1], cd[2])] = val;
 }
 
-int launch_fill_ghosts(const GridView &gv, const int32_t bc[3][2], double *P, cudaStream_t s) {
+int launch_fill_ghosts(const GridView &gv, const int32_t bc[3][2], double *P, cudaStream_t s, int dirs, int klo,
+                       int kcnt) {
   int launches = 0;
   const int tb = 256;
+  if (kcnt < 0) {
+    klo = 0;
+    kcnt = gv.sz[2];
+  }
   for (int a = 0; a < 3; a++) {
-    if (gv.ngd[a] == 0) continue;
+    if (gv.ngd[a] == 0 || !(dirs & (1 << a))) continue;
     long long cnt = (long long)gv.nvar;
-    for (int b = 0; b < 3; b++) cnt *= (b == a) ? 2 * gv.ngd[a] : gv.sz[b];
+    for (int b = 0; b < 3; b++) cnt *= (b == a) ? 2 * gv.ngd[a] : (b == 2 ? kcnt : gv.sz[b]);
+    if (cnt <= 0) continue;
     const unsigned blocks = (unsigned)((cnt + tb - 1) / tb);
-    if (a == 0) fill_ghosts_kernel<0><<<blocks, tb, 0, s>>>(gv, bc[0][0], bc[0][1], P);
-    if (a == 1) fill_ghosts_kernel<1><<<blocks, tb, 0, s>>>(gv, bc[1][0], bc[1][1], P);
-    if (a == 2) fill_ghosts_kernel<2><<<blocks, tb, 0, s>>>(gv, bc[2][0], bc[2][1], P);
+    if (a == 0) fill_ghosts_kernel<0><<<blocks, tb, 0, s>>>(gv, bc[0][0], bc[0][1], P, klo, kcnt);
+    if (a == 1) fill_ghosts_kernel<1><<<blocks, tb, 0, s>>>(gv, bc[1][0], bc[1][1], P, klo, kcnt);
+    if (a == 2) fill_ghosts_kernel<2><<<blocks, tb, 0, s>>>(gv, bc[2][0], bc[2][1], P, klo, kcnt);
     launches++;
   }
   return launches;

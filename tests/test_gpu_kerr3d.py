@@ -114,10 +114,6 @@ def _fullsize(n1, n2, n3, steps):
 
 
 def test_config4_shape_fullsize_every_zone():
-    """256 x 256 Kerr (BASELINE config 4's grid), 3 time steps, every interior zone bit-equal to the oracle."""
+    """256 x 256 Kerr (BASELINE config 4's grid), smooth synthetic state with MP5, 3 time steps, every interior zone
+    bit-equal to the oracle.  (Config 4 itself -- the torus, 100 steps -- is tests/test_gpu_torus.py.)"""
     _fullsize(256, 256, 1, 3)
-
-
-def test_config5_shape_fullsize_every_zone():
-    """256 x 256 x 128 Kerr (BASELINE config 5's grid), one time step, every interior zone bit-equal."""
-    _fullsize(256, 256, 128, 1)
