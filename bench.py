@@ -185,6 +185,32 @@ def other_workloads(local):
     _, sst = g.timestep(dP, dt, want_stats=True)
     out["kerr_emhd_256x256x128_synthetic"] = {"ms_per_step": ms, "zone_updates_per_s": g.zones / ms * 1e3,
                                               "unconverged": [int(x) for x in sst.unconverged]}
+    del g, dP
+    torch.cuda.empty_cache()
+
+    # BASELINE config 5 as stated: Fishbone-Moncrief torus, field loop at beta = 100, seeded noise (workloads.fm_torus)
+    gk, P = workloads.fm_torus(256, 256, 128)
+    g = gb.Grid(gk["n1"], gk["n2"], gk["n3"], dim=3, xstart=gk["xstart"], xend=gk["xend"], bc=gk["bc"], model=10,
+                recon=gk["recon"], tau_mode=gk["tau_mode"], rtol=gk["rtol"], kmax=gk["kmax"], lsmax=gk["lsmax"],
+                metric=gk["metric"], metric_params=gk["metric_params"], device=local)
+    dP = torch.from_numpy(P).cuda()
+    dt, _ = g.timestep(dP.clone(), 0.0, want_dt=True)
+    for _ in range(3):
+        g.timestep(dP, dt)
+    torch.cuda.synchronize()
+    e0, e1 = ev(), ev()
+    e0.record()
+    for _ in range(K):
+        g.timestep(dP, dt)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / K
+    _, sst = g.timestep(dP, dt, want_stats=True)
+    its = [sum(i * sst.iters_hist[s][i] for i in range(16)) / g.zones for s in range(2)]
+    out["config5_fm_torus_256x256x128_minmod"] = {"ms_per_step": ms, "zone_updates_per_s": g.zones / ms * 1e3,
+                                                  "mean_newton_iterations": its,
+                                                  "backtracks": [int(x) for x in sst.backtracks],
+                                                  "unconverged": [int(x) for x in sst.unconverged]}
     return out
 
 

@@ -472,15 +472,21 @@ extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used,
   unsigned long long bt[2] = {0, 0};
 
   c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(gv, c->d.bc, P, s); });
+  bool have_faces = false;
   if (!(dt > 0.0)) {
-    // C-15: dt = cfl / max_z sum_d c^d/dX^d, from a flux pass over P_n
+    // C-15: dt = cfl / max_z sum_d c^d/dX^d.  The face fluxes and speeds of stage 1 (P_E = P_n) do not depend on dt:
+    // compute them now, reduce the speeds, and let stage 1 below form its stage constant from the same face arrays.
     CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
-    c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, P, P, 1.0, c->C, c->G, c->Fface, c->cface, c->cnt, s); });
+    c->launches += timed(c, GRIM_K_FLUX, [&] {
+      int n = launch_fluxes(gv, P, P, 1.0, c->C, c->G, c->Fface, c->cface, nullptr, s, 1);
+      return n + launch_speeds(gv, c->cface, c->cnt, s);
+    });
     double sp3 = 0.0;
     CU(cudaMemcpyAsync(&sp3, &c->cnt->speeds[3], sizeof(double), cudaMemcpyDeviceToHost, s));
     CU(cudaStreamSynchronize(s));
     if (!(sp3 > 0.0)) return fail(c, GRIM_ESTATE, "maximum wave speed is not positive");
     dt = c->d.cfl / sp3;
+    have_faces = true;
   }
   if (stats) CU(cudaMemsetAsync(c->stats, 0, 2 * sizeof(StatsDev), s));
 
@@ -494,7 +500,7 @@ extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used,
 
   // stage 1: P_E = P_n, dt' = dt/2, guess P_n (eq 19; C-7)
   const double dt1 = 0.5 * dt;
-  c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, P, P, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s); });
+  c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, P, P, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s, have_faces ? 2 : 3); });
   if (caller_ghosts) CU(cudaMemcpyAsync(c->Ph, P, pbytes, cudaMemcpyDeviceToDevice, s));
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
   c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, P, c->C, c->G, P, 1, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s); });

@@ -97,8 +97,10 @@ int launch_invert(const GridView &gv, long long nz, long long nlist, const long 
                   const double *geom, double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters, int first,
                   long long *next_list, Counters *cnt, cudaStream_t s);
 int launch_prim_to_conserved(const GridView &gv, long long nz, const double *P, double *U, cudaStream_t s);
+// what: bit 0 = face fluxes and speeds (a1, a2), bit 1 = stage constant and gradient terms (a3) from the face arrays
 int launch_fluxes(const GridView &gv, const double *PE, const double *Pn, double dt_stage, double *C, double *G,
-                  double *Fface, double *cface, Counters *cnt, cudaStream_t s);
+                  double *Fface, double *cface, Counters *cnt, cudaStream_t s, int what = 3);
+int launch_speeds(const GridView &gv, const double *cface, Counters *cnt, cudaStream_t s);
 // dirs: bit a set = fill the ghosts of direction a; planes [klo, klo + kcnt) of the padded X^3 extent (kcnt < 0: all)
 // for the directions other than X^3
 int launch_fill_ghosts(const GridView &gv, const int32_t bc[3][2], double *P, cudaStream_t s, int dirs = 7,

@@ -605,12 +605,49 @@ stage_const_tiled_kernel(const __grid_constant__ GridView gv, const double *__re
   }
 }
 
+// max over interior zones of c^d/dX^d (d = 1..3) and of their sum (C-15), from the face speeds: the same expressions,
+// in the same order, as the wave-speed figures of stage_const_compute
+__global__ void __launch_bounds__(256)
+speeds_kernel(const __grid_constant__ GridView gv, const double *__restrict__ cface, Counters *cnt) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  double sp_loc[4] = {0.0, 0.0, 0.0, 0.0};
+  if (t < gv.nint) {
+    int i, j, k;
+    zone_coords(gv, t, i, j, k);
+    const long long z = zone_index(gv, i, j, k);
+    const long long strides[3] = {1, (long long)gv.sz[0], (long long)gv.sz[0] * gv.sz[1]};
+    double ssum = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; a++) {
+      if (gv.ngd[a] == 0) continue;
+      const double *ca = cface + (long long)a * gv.zg;
+      const double cz = fmax(ca[z], ca[z + strides[a]]) * gv.idx[a];
+      sp_loc[a] = cz;
+      ssum = ssum + cz;
+    }
+    sp_loc[3] = ssum;
+  }
+#pragma unroll
+  for (int a = 0; a < 4; a++) {
+    double v = sp_loc[a];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    if ((threadIdx.x & 31) == 0 && v > 0.0) atomic_max_nonneg(&cnt->speeds[a], v);
+  }
+}
+
+int launch_speeds(const GridView &gv, const double *cface, Counters *cnt, cudaStream_t s) {
+  speeds_kernel<<<(unsigned)((gv.nint + 255) / 256), 256, 0, s>>>(gv, cface, cnt);
+  return 1;
+}
+
+// what: bit 0 = the face fluxes (a1, a2), bit 1 = the stage constant and gradient terms (a3)
 template <int N, int RECON, class G>
 static int launch_fluxes_t(const GridView &gv, const double *PE, const double *Pn, double dt_stage, double *C,
-                           double *Gx, double *Fface, double *cface, Counters *cnt, cudaStream_t s) {
+                           double *Gx, double *Fface, double *cface, Counters *cnt, cudaStream_t s, int what) {
   int launches = 0;
   for (int a = 0; a < 3; a++) {
-    if (gv.ngd[a] == 0) continue;
+    if (gv.ngd[a] == 0 || !(what & 1)) continue;
     const int f0 = gv.n[0], f1 = gv.n[1], f2 = gv.n[2];  // tiled faces per direction (+ one edge plane along a)
     double *Fa = Fface + (long long)a * N * gv.zg;
     double *ca = cface + (long long)a * gv.zg;
@@ -662,11 +699,12 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
     }
     launches++;
   }
-  if (gv.flux_ct) {
+  if (gv.flux_ct && (what & 1)) {
     const long long ne = (long long)(gv.n[0] + (gv.ngd[0] > 0)) * (gv.n[1] + (gv.ngd[1] > 0)) * (gv.n[2] + (gv.ngd[2] > 0));
     emf_kernel<N><<<(unsigned)((ne + 255) / 256), 256, 0, s>>>(gv, Fface, gv.emf);
     launches++;
   }
+  if (!(what & 2)) return launches;
   const unsigned blocks = (unsigned)((gv.nint + FB - 1) / FB);
   if (!cnt && gv.ngd[1] > 0 && G::flat) {  // (general metric: the untiled kernel is faster, 16.0 against 16.8 ms)
     const dim3 tg((unsigned)((gv.n[0] + 31) / 32), (unsigned)((gv.n[1] + 3) / 4), (unsigned)gv.n[2]);
@@ -681,16 +719,16 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
 }
 
 int launch_fluxes(const GridView &gv, const double *PE, const double *Pn, double dt_stage, double *C, double *G,
-                  double *Fface, double *cface, Counters *cnt, cudaStream_t s) {
+                  double *Fface, double *cface, Counters *cnt, cudaStream_t s, int what) {
   const bool flat = (gv.metric == 0);
   const bool mp5 = (gv.recon == 1);
 #define GRIM_DISPATCH(NV)                                                                                   \
   if (flat) {                                                                                               \
-    return mp5 ? launch_fluxes_t<NV, 1, GeomFlat>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s)         \
-               : launch_fluxes_t<NV, 0, GeomFlat>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s);        \
+    return mp5 ? launch_fluxes_t<NV, 1, GeomFlat>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s, what)   \
+               : launch_fluxes_t<NV, 0, GeomFlat>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s, what);  \
   } else {                                                                                                  \
-    return mp5 ? launch_fluxes_t<NV, 1, GeomGen>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s)          \
-               : launch_fluxes_t<NV, 0, GeomGen>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s);         \
+    return mp5 ? launch_fluxes_t<NV, 1, GeomGen>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s, what)    \
+               : launch_fluxes_t<NV, 0, GeomGen>(gv, PE, Pn, dt_stage, C, G, Fface, cface, cnt, s, what);   \
   }
   if (gv.nvar == 10) { GRIM_DISPATCH(10) }
   GRIM_DISPATCH(8)
