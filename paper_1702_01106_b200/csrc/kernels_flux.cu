@@ -12,9 +12,12 @@
 //   emf_kernel            : flux-CT, face -> edge averages (L327-335).
 //   stage_const_kernel    : one thread per interior zone; differences the face fluxes, adds -U(P_n)/dt' and the
 //                           explicit sources, limited slopes of the derived quantities, max wave-speed figures.
+#include <type_traits>
+
 #include "grim_internal.h"
 #include "problems.cuh"
 #include "recon.cuh"
+#include "tma.cuh"
 
 namespace grim {
 
@@ -163,6 +166,98 @@ face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__
     cface[z] = c;
   } else {
     face_replay<N, RECON, G, DIR>(gv, PE, z, i, j, Fface, cface);
+  }
+}
+
+// The same tiles with the stencil zones brought in by TMA, one tile ahead of the arithmetic.  A block is persistent: it
+// takes the tiles b, b + gridDim.x, ...; while it computes the faces of one tile from buffer q, the bulk tensor copy of
+// the next tile's box -- all N variables, (T0 + halo) x (T1 + halo) x (T2 + halo) zones, out-of-range zones read as
+// zero -- lands in buffer 1 - q and signals that buffer's mbarrier.  One thread issues the copy; nobody computes
+// addresses or holds staging registers.  (A TMA box row starts on a 16-byte boundary and is a multiple of 16 bytes long:
+// the box starts at the even X^1 index at or below the first stencil zone and has an even X^1 extent.)
+#ifndef GRIM_FLUX_TMA
+#define GRIM_FLUX_TMA 1
+#endif
+// blocks per resident block slot: 1 = fully persistent; 0 = one tile per block (no prefetch, the copy only replaces the
+// per-thread staging loads)
+#ifndef GRIM_FLUX_TMA_WAVES
+#define GRIM_FLUX_TMA_WAVES 0
+#endif
+template <int RECON, int DIR>
+struct TmaTile {
+  using T = FaceTile<DIR>;
+  static constexpr int H = (RECON == 1) ? 6 : 4, LO = H / 2;
+  // one more zone than the stencil needs, rounded up to even: the box starts at an even X^1 index (see below)
+  static constexpr int E0 = (T::T0 + (DIR == 0 ? H - 1 : 0) + 2) / 2 * 2, E1 = T::T1 + (DIR == 1 ? H - 1 : 0),
+                       E2 = T::T2 + (DIR == 2 ? H - 1 : 0), EZ = E0 * E1 * E2;
+  static constexpr int MS = (DIR == 0) ? 1 : (DIR == 1) ? E0 : E0 * E1;
+};
+template <int N, int RECON, int DIR>
+__host__ __device__ constexpr size_t tma_tile_bytes() {
+  return ((size_t)N * TmaTile<RECON, DIR>::EZ * sizeof(double) + 127) / 128 * 128;
+}
+
+template <int N, int RECON, class G, int DIR>
+__global__ void __launch_bounds__(FB, G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN)
+face_flux_tma_kernel(const __grid_constant__ GridView gv, const __grid_constant__ CUtensorMap tmap,
+                     const double *__restrict__ PE, double *__restrict__ Fface, double *__restrict__ cface, int ntx,
+                     int nty, int ntz) {
+  using T = FaceTile<DIR>;
+  using X = TmaTile<RECON, DIR>;
+  constexpr uint32_t BYTES = (uint32_t)(N * X::EZ * sizeof(double));
+  extern __shared__ __align__(128) unsigned char tma_smem[];
+  __shared__ uint64_t bar[2];
+  double *buf[2] = {(double *)tma_smem,
+                    (double *)(tma_smem + (GRIM_FLUX_TMA_WAVES == 0 ? 0 : tma_tile_bytes<N, RECON, DIR>()))};
+  const long long ntiles = (long long)ntx * nty * ntz;
+  if (threadIdx.x == 0) {
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    mbar_init_fence();
+  }
+  __syncthreads();
+  auto origin = [&](long long tile, int &fi, int &fj, int &fk) {
+    const unsigned tl = (unsigned)tile, nx = (unsigned)ntx, ny = (unsigned)nty;  // (the tile count fits 32 bits)
+    const int tx = (int)(tl % nx), ty = (int)((tl / nx) % ny), tz = (int)(tl / (nx * ny));
+    fi = gv.ngd[0] + tx * T::T0;
+    fj = gv.ngd[1] + ty * T::T1;
+    fk = gv.ngd[2] + gv.koff + tz * T::T2;
+  };
+  auto issue = [&](long long tile, int q) {  // one thread
+    int fi, fj, fk;
+    origin(tile, fi, fj, fk);
+    mbar_expect_tx(&bar[q], BYTES);
+    tma_load_4d(buf[q], &tmap, &bar[q], (fi - (DIR == 0 ? X::LO : 0)) & ~1, fj - (DIR == 1 ? X::LO : 0),
+                fk - (DIR == 2 ? X::LO : 0), 0);
+  };
+  const int xshift = (gv.ngd[0] - (DIR == 0 ? X::LO : 0)) & 1;  // tile origins advance by an even T0
+  const int t0 = (int)threadIdx.x % T::T0, t1 = ((int)threadIdx.x / T::T0) % T::T1,
+            t2 = (int)threadIdx.x / (T::T0 * T::T1);
+  if (threadIdx.x == 0 && (long long)blockIdx.x < ntiles) issue(blockIdx.x, 0);
+  int it = 0;
+  for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
+    const int q = it & 1;
+    // buffer 1 - q was released by the block-wide sync that ended the previous iteration
+    if (threadIdx.x == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x, q ^ 1);
+    mbar_wait(&bar[q], (uint32_t)((it >> 1) & 1));
+    int fi, fj, fk;
+    origin(tile, fi, fj, fk);
+    const int i = fi + t0, j = fj + t1, k = fk + t2;
+    if (i < gv.ngd[0] + gv.n[0] && j < gv.ngd[1] + gv.n[1] && k < gv.ngd[2] + gv.koff + gv.n[2]) {
+      const long long z = zone_index(gv, i, j, k);
+      SpecArith ar;
+      double F[N], c;
+      const TileStencil<X::EZ, X::MS> st{buf[q] + (t2 * X::E1 + t1) * X::E0 + t0 + xshift};
+      face_compute<N, RECON, G, DIR>(ar, gv, st, i, j, F, c);
+      if (ar.good()) {
+#pragma unroll
+        for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
+        cface[z] = c;
+      } else {
+        face_replay<N, RECON, G, DIR>(gv, PE, z, i, j, Fface, cface);
+      }
+    }
+    __syncthreads();
   }
 }
 
@@ -654,9 +749,37 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
     auto tiles = [&](int t0, int t1, int t2) {
       return dim3((unsigned)((f0 + t0 - 1) / t0), (unsigned)((f1 + t1 - 1) / t1), (unsigned)((f2 + t2 - 1) / t2));
     };
-    if (a == 0) face_flux_kernel<N, RECON, G, 0><<<tiles(128, 1, 1), FB, 0, s>>>(gv, PE, Fa, ca);
-    if (a == 1) face_flux_kernel<N, RECON, G, 1><<<tiles(32, 4, 1), FB, 0, s>>>(gv, PE, Fa, ca);
-    if (a == 2) face_flux_kernel<N, RECON, G, 2><<<tiles(32, 1, 4), FB, 0, s>>>(gv, PE, Fa, ca);
+    bool by_tma = false;
+#if GRIM_FLUX_TMA
+    {
+      auto tma = [&](auto dirc) {
+        constexpr int D = decltype(dirc)::value;
+        using X = TmaTile<RECON, D>;
+        using T = FaceTile<D>;
+        CUtensorMap map;
+        if (!make_tile_map(&map, PE, gv.sz[0], gv.sz[1], gv.sz[2], N, gv.zg, X::E0, X::E1, X::E2)) return false;
+        const dim3 tg = tiles(T::T0, T::T1, T::T2);
+        const long long nt = (long long)tg.x * tg.y * tg.z;
+        const size_t smem = (GRIM_FLUX_TMA_WAVES == 0 ? 1 : 2) * tma_tile_bytes<N, RECON, D>();
+        auto kern = face_flux_tma_kernel<N, RECON, G, D>;
+        cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        const int per_sm = G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN;
+        long long blocks = (long long)per_sm * (gv.nsm > 0 ? gv.nsm : 148) * GRIM_FLUX_TMA_WAVES;
+        if (blocks > nt || GRIM_FLUX_TMA_WAVES == 0) blocks = nt;
+        if (nt >= (1LL << 31)) return false;
+        kern<<<(unsigned)blocks, FB, smem, s>>>(gv, map, PE, Fa, ca, (int)tg.x, (int)tg.y, (int)tg.z);
+        return true;
+      };
+      if (a == 0) by_tma = tma(std::integral_constant<int, 0>());
+      if (a == 1) by_tma = tma(std::integral_constant<int, 1>());
+      if (a == 2) by_tma = tma(std::integral_constant<int, 2>());
+    }
+#endif
+    if (!by_tma) {
+      if (a == 0) face_flux_kernel<N, RECON, G, 0><<<tiles(128, 1, 1), FB, 0, s>>>(gv, PE, Fa, ca);
+      if (a == 1) face_flux_kernel<N, RECON, G, 1><<<tiles(32, 4, 1), FB, 0, s>>>(gv, PE, Fa, ca);
+      if (a == 2) face_flux_kernel<N, RECON, G, 2><<<tiles(32, 1, 4), FB, 0, s>>>(gv, PE, Fa, ca);
+    }
     // what the tiles leave: the upper boundary plane along a, and with flux-CT one layer of faces in every active
     // transverse ghost direction (the edge averages reach there)
     auto box = [&](const FaceBox &bx) {
