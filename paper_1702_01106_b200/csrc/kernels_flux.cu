@@ -700,6 +700,82 @@ stage_const_tiled_kernel(const __grid_constant__ GridView gv, const double *__re
   }
 }
 
+// The tiled stage-constant kernel with its three face-flux tiles brought in by TMA (one 4-D box per direction, all N
+// variables): rows of W = T0 + 2 faces starting at the even X^1 index at or below the tile's first face.
+template <int N, int T0, int T1>
+struct TileFluxTma {
+  static constexpr int W = T0 + 2;
+  static constexpr int S0 = W * T1, S1 = W * (T1 + 1), S2 = 2 * W * T1;
+  // offsets of the three boxes in doubles, each on a 128-byte boundary (TMA destination)
+  static constexpr int O1 = (N * S0 + 15) / 16 * 16, O2 = (O1 + N * S1 + 15) / 16 * 16;
+  static constexpr int SIZE = O2 + N * S2;
+  const double *s;
+  int t0, t1;  // t0 includes the shift of the box start
+  __device__ __forceinline__ double operator()(int a, int v, int up) const {
+    if (a == 0) return s[v * S0 + t1 * W + t0 + up];
+    if (a == 1) return s[O1 + v * S1 + (t1 + up) * W + t0];
+    return s[O2 + v * S2 + up * W * T1 + t1 * W + t0];
+  }
+};
+
+struct FluxMaps {
+  CUtensorMap m[3];
+};
+
+template <int N, class G, bool CT>
+__global__ void __launch_bounds__(FB, G::flat ? GRIM_SC_MINB : GRIM_SC_MINB_GEN)
+stage_const_tma_kernel(const __grid_constant__ GridView gv, const __grid_constant__ FluxMaps maps,
+                       const double *__restrict__ PE, const double *__restrict__ Pn, double dt_stage,
+                       const double *__restrict__ Fface, const double *__restrict__ cface, double *__restrict__ C,
+                       double *__restrict__ Gx) {
+  constexpr int T0 = 32, T1 = 4;
+  using TF = TileFluxTma<N, T0, T1>;
+  extern __shared__ __align__(128) unsigned char sc_smem[];
+  __shared__ uint64_t bar;
+  double *tile = (double *)sc_smem;
+  const int i0 = gv.ngd[0] + (int)blockIdx.x * T0, j0 = gv.ngd[1] + (int)blockIdx.y * T1,
+            k = gv.ngd[2] + gv.koff + (int)blockIdx.z;
+  const long long zg = gv.zg;
+  if (threadIdx.x == 0) {
+    mbar_init(&bar, 1);
+    mbar_init_fence();
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    const bool d3 = gv.ngd[2] > 0;
+    mbar_expect_tx(&bar, (uint32_t)(N * (TF::S0 + TF::S1 + (d3 ? TF::S2 : 0)) * sizeof(double)));
+    tma_load_4d(tile, &maps.m[0], &bar, i0 & ~1, j0, k, 0);
+    tma_load_4d(tile + TF::O1, &maps.m[1], &bar, i0 & ~1, j0, k, 0);
+    if (d3) tma_load_4d(tile + TF::O2, &maps.m[2], &bar, i0 & ~1, j0, k, 0);
+  }
+  // the zone's own primitives are requested while the tiles are in flight
+  const int t0 = (int)threadIdx.x % T0, t1 = (int)threadIdx.x / T0;
+  const int i = i0 + t0, j = j0 + t1;
+  const bool valid = i < gv.ngd[0] + gv.n[0] && j < gv.ngd[1] + gv.n[1];
+  const long long z = zone_index(gv, valid ? i : gv.ngd[0], valid ? j : gv.ngd[1], k);
+  double Pn_z[N], PE_z[N];
+#pragma unroll
+  for (int v = 0; v < N; v++) {
+    Pn_z[v] = Pn[v * zg + z];
+    PE_z[v] = PE[v * zg + z];
+  }
+  mbar_wait(&bar, 0);
+  if (!valid) return;
+  const long long id = (long long)j * gv.sz[0] + i;
+  double Cout[N], Gout[3] = {0.0, 0.0, 0.0}, sp_loc[4];
+  SpecArith ar;
+  const TF fs{tile, t0 + (i0 & 1), t1};
+  stage_const_compute<N, G, CT>(ar, gv, fs, Pn_z, PE_z, PE, Pn, dt_stage, Fface, cface, false, z, id, Cout, Gout,
+                                sp_loc);
+  if (!ar.good()) stage_const_replay<N, G, CT>(gv, PE, Pn, dt_stage, Fface, cface, false, z, id, Cout, Gout, sp_loc);
+#pragma unroll
+  for (int v = 0; v < N; v++) C[v * zg + z] = Cout[v];
+  if constexpr (N == 10) {
+#pragma unroll
+    for (int v = 0; v < 3; v++) Gx[v * zg + z] = Gout[v];
+  }
+}
+
 // max over interior zones of c^d/dX^d (d = 1..3) and of their sum (C-15), from the face speeds: the same expressions,
 // in the same order, as the wave-speed figures of stage_const_compute
 __global__ void __launch_bounds__(256)
@@ -831,7 +907,36 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
   const unsigned blocks = (unsigned)((gv.nint + FB - 1) / FB);
   if (!cnt && gv.ngd[1] > 0 && G::flat) {  // (general metric: the untiled kernel is faster, 16.0 against 16.8 ms)
     const dim3 tg((unsigned)((gv.n[0] + 31) / 32), (unsigned)((gv.n[1] + 3) / 4), (unsigned)gv.n[2]);
-    if (gv.flux_ct) stage_const_tiled_kernel<N, G, true><<<tg, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx);
+    bool by_tma = false;
+#if GRIM_FLUX_TMA
+    {
+      using TF = TileFluxTma<N, 32, 4>;
+      FluxMaps maps;
+      bool ok = true;
+      const int b1[3] = {4, 5, 4}, b2[3] = {1, 1, 2};
+      for (int a = 0; a < 3 && ok; a++) {
+        if (gv.ngd[a] == 0) {
+          maps.m[a] = maps.m[0];
+          continue;
+        }
+        ok = make_tile_map(&maps.m[a], Fface + (long long)a * N * gv.zg, gv.sz[0], gv.sz[1], gv.sz[2], N, gv.zg, TF::W,
+                           b1[a], b2[a]);
+      }
+      if (ok) {
+        const size_t smem = (size_t)TF::SIZE * sizeof(double);
+        if (gv.flux_ct) {
+          cudaFuncSetAttribute(stage_const_tma_kernel<N, G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+          stage_const_tma_kernel<N, G, true><<<tg, FB, smem, s>>>(gv, maps, PE, Pn, dt_stage, Fface, cface, C, Gx);
+        } else {
+          cudaFuncSetAttribute(stage_const_tma_kernel<N, G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+          stage_const_tma_kernel<N, G, false><<<tg, FB, smem, s>>>(gv, maps, PE, Pn, dt_stage, Fface, cface, C, Gx);
+        }
+        by_tma = true;
+      }
+    }
+#endif
+    if (by_tma) {
+    } else if (gv.flux_ct) stage_const_tiled_kernel<N, G, true><<<tg, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx);
     else stage_const_tiled_kernel<N, G, false><<<tg, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx);
   } else if (gv.flux_ct) {
     stage_const_kernel<N, G, true><<<blocks, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx, cnt);
