@@ -53,6 +53,13 @@ struct grim_ctx {
   long long invbuf_nz;
   int64_t launches;
   int no_pipeline;             // GRIM_HOST_PIPELINE=0 in the environment: grim_timestep_host copies, steps, copies
+  // sweep policy of solve_stage: the deferred-zone counts of the recent sweep-mode solves arrive asynchronously in
+  // pinned host memory; a run whose solves never defer a zone (smooth data) goes back to single launches and probes again
+  // every GRIM_SWEEP_PROBE solves
+  unsigned long long *sweep_counts;  // pinned, SWEEP_RING entries
+  cudaEvent_t sweep_ev[4];
+  int sweep_pending[4];
+  int sweep_slot, sweep_quiet, sweep_skip;
   // optional per-kernel-class timing (grim_set_timing): event pairs recorded around the launches
   int timing;
   std::vector<KernelSpan> spans;
@@ -159,6 +166,10 @@ extern "C" void grim_free(grim_ctx *c) {
     if (p) cudaFree(p);
   for (auto e : c->ev_in) cudaEventDestroy(e);
   for (auto e : c->ev_done) cudaEventDestroy(e);
+  if (c->sweep_counts) {
+    cudaFreeHost(c->sweep_counts);
+    for (int q = 0; q < 4; q++) cudaEventDestroy(c->sweep_ev[q]);
+  }
   if (c->s_in) cudaStreamDestroy(c->s_in);
   if (c->s_out) cudaStreamDestroy(c->s_out);
   delete c;
@@ -391,6 +402,83 @@ extern "C" int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_
   return GRIM_OK;
 }
 
+// A fresh solve of every interior zone to a terminal status (steps a4-a7), in sweeps: the first launch gives every zone
+// GRIM_STAGE_SWEEP iterations; the zones that need more -- a few per cent in a run whose iteration counts spread (the
+// torus: 2-8), none in a smooth run -- are collected and solved afresh, to the end, by a second launch over that list
+// only, so that a warp does not idle through the long solves of a few of its lanes.  The per-zone results are those of
+// one uninterrupted solve (it IS one, for every zone); the list length stays on the device.
+#ifndef GRIM_STAGE_SWEEP
+#define GRIM_STAGE_SWEEP 4
+#endif
+#ifndef GRIM_SWEEP_PROBE
+#define GRIM_SWEEP_PROBE 64
+#endif
+static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const double *PE, const double *C,
+                       const double *G, const double *Pguess, double dt_stage, double *Pout, double *resnorm,
+                       int32_t *status, int32_t *iters) {
+  cudaStream_t s = c->stream;
+  bool sweeps = GRIM_STAGE_SWEEP > 0 && gv.sp.kmax > GRIM_STAGE_SWEEP;
+  if (sweeps) {
+    // Both modes give the same results zone for zone; the policy only decides which is faster.  Collect the counts of
+    // earlier sweep-mode solves that have landed: 4 in a row without a deferred zone -> single launches for a while.
+    if (!c->sweep_counts) {
+      CU(cudaMallocHost((void **)&c->sweep_counts, 4 * sizeof(unsigned long long)));
+      for (int q = 0; q < 4; q++) {
+        CU(cudaEventCreateWithFlags(&c->sweep_ev[q], cudaEventDisableTiming));
+        c->sweep_pending[q] = 0;
+      }
+    }
+    for (int q = 0; q < 4; q++) {
+      if (c->sweep_pending[q] && cudaEventQuery(c->sweep_ev[q]) == cudaSuccess) {
+        c->sweep_pending[q] = 0;
+        if (c->sweep_counts[q] == 0) c->sweep_quiet++;
+        else c->sweep_quiet = 0;
+      }
+    }
+    if (c->sweep_quiet >= 4) {
+      c->sweep_quiet = 0;
+      c->sweep_skip = GRIM_SWEEP_PROBE;
+    }
+    if (c->sweep_skip > 0) {
+      c->sweep_skip--;
+      sweeps = false;
+    }
+  }
+  if (sweeps && c->list_cap < gv.nint) {
+    for (int a = 0; a < 2; a++) {
+      if (c->list[a]) cudaFree(c->list[a]);
+      c->list[a] = nullptr;
+      CU(cudaMalloc((void **)&c->list[a], (size_t)gv.nint * sizeof(long long)));
+    }
+    c->list_cap = gv.nint;
+  }
+  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
+  GridView g1 = gv;
+  if (sweeps) g1.sp.kmax = GRIM_STAGE_SWEEP;
+  c->launches += timed(c, GRIM_K_NEWTON, [&] {
+    return launch_newton_stage(g1, Pn, PE, C, G, Pguess, 1, dt_stage, 0, Pout, resnorm, status, iters, c->cnt, s, nullptr, 0,
+                               sweeps ? c->list[0] : nullptr);
+  });
+  int rc = check_launch(c, "newton_stage kernel");
+  if (rc || !sweeps) return rc;
+  // the second sweep reads the list length from the device: no synchronisation; the length also goes to the host,
+  // asynchronously, for the sweep policy
+  {
+    const int q = c->sweep_slot;
+    if (!c->sweep_pending[q]) {
+      CU(cudaMemcpyAsync(&c->sweep_counts[q], &c->cnt->list_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
+      CU(cudaEventRecord(c->sweep_ev[q], s));
+      c->sweep_pending[q] = 1;
+      c->sweep_slot = (q + 1) % 4;
+    }
+  }
+  c->launches += timed(c, GRIM_K_NEWTON, [&] {
+    return launch_newton_stage(gv, Pn, PE, C, G, Pguess, 1, dt_stage, 0, Pout, resnorm, status, iters, c->cnt, s,
+                               c->list[0], 0, nullptr);
+  });
+  return check_launch(c, "newton_stage kernel (second sweep)");
+}
+
 extern "C" int grim_newton_solve(grim_ctx *c, const double *P_n, const double *P_E, const double *C, const double *G,
                                  double dt_stage, const double *P_guess, double *P_out, double *resnorm,
                                  int32_t *status, int32_t *iters) {
@@ -399,13 +487,8 @@ extern "C" int grim_newton_solve(grim_ctx *c, const double *P_n, const double *P
   if (!P_n || !P_E || !P_guess || !P_out) return fail(c, GRIM_EINVAL, "grim_newton_solve: null array argument");
   if (!(dt_stage > 0.0)) return fail(c, GRIM_EINVAL, "dt_stage must be positive");
   CU(cudaSetDevice(c->d.device));
-  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
-  c->launches += timed(c, GRIM_K_NEWTON, [&] {
-    return launch_newton_stage(c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, P_guess, 1, dt_stage, 0, P_out,
-                               resnorm ? resnorm : c->resnorm, status ? status : c->status,
-                               iters ? iters : c->iters, c->cnt, c->stream);
-  });
-  return check_launch(c, "newton_stage kernel");
+  return solve_stage(c, c->gv, P_n, P_E, C ? C : c->C, G ? G : c->G, P_guess, dt_stage, P_out,
+                     resnorm ? resnorm : c->resnorm, status ? status : c->status, iters ? iters : c->iters);
 }
 
 extern "C" int grim_prim_to_conserved(grim_ctx *c, int64_t nz, const double *P, double *U) {
@@ -502,8 +585,8 @@ extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used,
   const double dt1 = 0.5 * dt;
   c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, P, P, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s, have_faces ? 2 : 3); });
   if (caller_ghosts) CU(cudaMemcpyAsync(c->Ph, P, pbytes, cudaMemcpyDeviceToDevice, s));
-  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
-  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, P, c->C, c->G, P, 1, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s); });
+  rc = solve_stage(c, gv, P, P, c->C, c->G, P, dt1, c->Ph, c->resnorm, c->status, c->iters);
+  if (rc) return rc;
   if (stats) {
     c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_stats(gv, P, dt1, c->resnorm, c->status, c->iters, &c->stats[0], s); });
     CU(cudaMemcpyAsync(&bt[0], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));
@@ -513,10 +596,9 @@ extern "C" int grim_timestep(grim_ctx *c, double *P, double dt, double *dt_used,
   c->launches += timed(c, GRIM_K_GHOSTS, [&] { return launch_fill_ghosts(gv, c->d.bc, c->Ph, s); });
   c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(gv, c->Ph, P, dt, c->C, c->G, c->Fface, c->cface, nullptr, s); });
   if (stats) CU(cudaStreamSynchronize(s));  // bt[0] must land before the counters are cleared
-  CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
   double *out2 = stats ? c->Pnew : P;
-  c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(gv, P, c->Ph, c->C, c->G, c->Ph, 1, dt, 0, out2, c->resnorm, c->status, c->iters,
-                                     c->cnt, s); });
+  rc = solve_stage(c, gv, P, c->Ph, c->C, c->G, c->Ph, dt, out2, c->resnorm, c->status, c->iters);
+  if (rc) return rc;
   if (stats) {
     c->launches += timed(c, GRIM_K_OTHER, [&] { return launch_stats(gv, P, dt, c->resnorm, c->status, c->iters, &c->stats[1], s); });
     CU(cudaMemcpyAsync(&bt[1], &c->cnt->backtracks, 8, cudaMemcpyDeviceToHost, s));

@@ -92,7 +92,8 @@ __device__ __forceinline__ void load_geom(const double *__restrict__ tab, long l
 // ---- kernel launchers (defined in the kernels_*.cu files); all enqueue on `s` and return the launch count ----
 int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *G,
                         const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
-                        int32_t *iters, Counters *cnt, cudaStream_t s);
+                        int32_t *iters, Counters *cnt, cudaStream_t s, const long long *list = nullptr,
+                        long long nlist = 0, long long *next_list = nullptr);
 int launch_invert(const GridView &gv, long long nz, long long nlist, const long long *list, const double *Ustar,
                   const double *geom, double *P, int32_t *iters, int32_t *status, double *resnorm, int max_iters, int first,
                   long long *next_list, Counters *cnt, cudaStream_t s);

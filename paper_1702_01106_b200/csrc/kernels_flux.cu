@@ -579,6 +579,9 @@ __device__ __noinline__ void stage_const_replay(const GridView &gv, const double
 #ifndef GRIM_SC_MINB
 #define GRIM_SC_MINB 4
 #endif
+#ifndef GRIM_SC_TILED_GEN
+#define GRIM_SC_TILED_GEN 1  // general metric: tiled (TMA) stage-constant kernel as well
+#endif
 #ifndef GRIM_SC_MINB_GEN
 #define GRIM_SC_MINB_GEN 2  // general metric: connection contractions, 6 neighbour geometries -> 255 registers
 #endif
@@ -905,7 +908,7 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
   }
   if (!(what & 2)) return launches;
   const unsigned blocks = (unsigned)((gv.nint + FB - 1) / FB);
-  if (!cnt && gv.ngd[1] > 0 && G::flat) {  // (general metric: the untiled kernel is faster, 16.0 against 16.8 ms)
+  if (!cnt && gv.ngd[1] > 0 && (G::flat || GRIM_SC_TILED_GEN)) {
     const dim3 tg((unsigned)((gv.n[0] + 31) / 32), (unsigned)((gv.n[1] + 3) / 4), (unsigned)gv.n[2]);
     bool by_tma = false;
 #if GRIM_FLUX_TMA

@@ -20,12 +20,18 @@ struct StageArgs {
   int fresh;             // != 0: a new solve; status and iters start at zero without being read
   double *Piter, *resnorm;
   int32_t *status, *iters;
+  // Active-set sweeps (SURVEY 7.2 "Divergence"): with next_list set (and kmax lowered to the sweep length by the
+  // caller), a zone that stops at kmax stores NOTHING and its interior index is appended to next_list
+  // (cnt->list_count); a later launch over that list (list != null) solves it afresh with the real kmax.
+  const long long *list;
+  long long nlist;
+  long long *next_list;
 };
 
 // One zone of one stage under arithmetic policy A: loads, set-up, Newton iteration, stores.  Returns false
 // WITHOUT storing when a speculative operation saw an operand outside its safe range (fp64ops.cuh); the caller
 // then replays the zone with ExactArith.  Otherwise packs (rejected line-search trials << 1) | still-active.
-template <int N, class G, bool RED, class A>
+template <int N, class G, bool RED, bool APPEND, class A>
 __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const StageArgs &a, long long z, int i, int j,
                                           int st, double *sj) {
   constexpr int M = Unknowns<N, RED>::M;
@@ -77,6 +83,9 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
   JacView<M, NB> jac{sj};
   double rn = newton_zone<N, RED, NB>(ar, prob, gv.sp, tol, P, it, st, a.max_iters, jac, nbt, &pc0);
   if (!ar.good()) return -1;
+  // first sweep (launched with kmax = the sweep length): a zone that ran out of iterations is deferred to the next
+  // sweep -- nothing stored, nothing counted
+  if (APPEND && (st & ST_KMAX)) return 1;
 #pragma unroll
   for (int v = 0; v < N; v++) a.Piter[v * gv.zg + z] = P[v];
   a.resnorm[z] = rn;
@@ -85,11 +94,11 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
   return (nbt << 1) | ((st & ST_TERMINAL) ? 0 : 1);
 }
 
-template <int N, class G, bool RED>
+template <int N, class G, bool RED, bool APPEND>
 __device__ __noinline__ int stage_zone_replay(const GridView &gv, const StageArgs &a, long long z, int i, int j,
                                               int st, double *sj) {
   ExactArith ar;
-  return stage_zone<N, G, RED>(ar, gv, a, z, i, j, st, sj);
+  return stage_zone<N, G, RED, APPEND>(ar, gv, a, z, i, j, st, sj);
 }
 
 #ifndef GRIM_N8_MINB
@@ -98,23 +107,43 @@ __device__ __noinline__ int stage_zone_replay(const GridView &gv, const StageArg
 #ifndef GRIM_RED_MINB
 #define GRIM_RED_MINB 2  // reduced solve: (N-3)^2 + N doubles of shared memory per zone leave room for 3 blocks
 #endif
-template <int N, class G, bool RED>
-__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB))
-newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
-  extern __shared__ double smem[];
-  const long long t = (long long)blockIdx.x * NB + threadIdx.x;
+// One thread's zone of a launch: interior zone zt (have = false: the thread has none).  Returns the packed result of
+// stage_zone with the deferred zones appended to a.next_list and removed from the count.
+template <int N, class G, bool RED, bool APPEND>
+__device__ __forceinline__ int stage_thread(const GridView &gv, const StageArgs &a, Counters *cnt, long long zt, bool have,
+                                            double *sj) {
   int res = 0;
-  if (t < gv.nint) {
+  if (have) {
     int i, j, k;
-    zone_coords(gv, t, i, j, k);
+    zone_coords(gv, zt, i, j, k);
     const long long z = zone_index(gv, i, j, k);
     const int st = a.fresh ? 0 : a.status[z];
     if (!(st & ST_TERMINAL)) {
       SpecArith ar;
-      res = stage_zone<N, G, RED>(ar, gv, a, z, i, j, st, smem + threadIdx.x);
-      if (res < 0) res = stage_zone_replay<N, G, RED>(gv, a, z, i, j, st, smem + threadIdx.x);
+      res = stage_zone<N, G, RED, APPEND>(ar, gv, a, z, i, j, st, sj);
+      if (res < 0) res = stage_zone_replay<N, G, RED, APPEND>(gv, a, z, i, j, st, sj);
     }
   }
+  if constexpr (APPEND) {
+    // warp-aggregated append of the deferred zones (order not deterministic; the per-zone results are)
+    const unsigned ballot = __ballot_sync(0xffffffffu, res & 1);
+    const int lane = threadIdx.x & 31;
+    unsigned long long base = 0;
+    if (lane == 0 && ballot) base = atomicAdd(&cnt->list_count, (unsigned long long)__popc(ballot));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (res & 1) a.next_list[base + __popc(ballot & ((1u << lane) - 1u))] = zt;
+    res &= ~1;
+  }
+  return res;
+}
+
+// APPEND: first sweep (zones that stop at the lowered kmax are deferred to a.next_list)
+template <int N, class G, bool RED, bool APPEND>
+__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB))
+newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
+  extern __shared__ double smem[];
+  const long long t = (long long)blockIdx.x * NB + threadIdx.x;
+  const int res = stage_thread<N, G, RED, APPEND>(gv, a, cnt, t, t < gv.nint, smem + threadIdx.x);
   // warp-aggregated counters
   unsigned long long na = __reduce_add_sync(0xffffffffu, (unsigned)(res & 1));
   unsigned long long nb = __reduce_add_sync(0xffffffffu, (unsigned)(res >> 1));
@@ -124,26 +153,65 @@ newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__
   }
 }
 
+// The launch over a list of deferred zones whose length is on the device (cnt->list_count, written by the launch
+// before): a resident grid of blocks strides over the list, so that the host need not know the length.
+template <int N, class G, bool RED>
+__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB))
+newton_stage_list_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
+  extern __shared__ double smem[];
+  const long long nlist = (long long)cnt->list_count;
+  unsigned n_act = 0, n_bt = 0;
+  for (long long t0 = (long long)blockIdx.x * NB; t0 < nlist; t0 += (long long)gridDim.x * NB) {
+    const long long t = t0 + threadIdx.x;
+    const bool have = t < nlist;
+    const int res = stage_thread<N, G, RED, false>(gv, a, cnt, have ? a.list[t] : 0, have, smem + threadIdx.x);
+    n_act += (unsigned)(res & 1);
+    n_bt += (unsigned)(res >> 1);
+  }
+  unsigned long long na = __reduce_add_sync(0xffffffffu, n_act);
+  unsigned long long nb = __reduce_add_sync(0xffffffffu, n_bt);
+  if ((threadIdx.x & 31) == 0) {
+    if (na) atomicAdd(&cnt->n_active, na);
+    if (nb) atomicAdd(&cnt->backtracks, nb);
+  }
+}
+
 template <int N, class G, bool RED>
 static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *Gx,
                           const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
-                          int32_t *iters, Counters *cnt, cudaStream_t s) {
+                          int32_t *iters, Counters *cnt, cudaStream_t s, const long long *list, long long nlist,
+                          long long *next_list) {
   constexpr int M = Unknowns<N, RED>::M;
   const size_t smem = (size_t)(M * M + N) * NB * sizeof(double);  // Jacobian + C per thread
   // per device and context, so set before every launch (cheap); a failure surfaces as the launch error
-  cudaFuncSetAttribute(newton_stage_kernel<N, G, RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  const StageArgs a{Pn, PE, C, Gx, Pguess, dt_stage, max_iters, fresh, Piter, resnorm, status, iters, list, nlist, next_list};
+  if (list) {
+    // the list's length is cnt->list_count on the device: a resident grid strides over it (nothing to do: ~5 us)
+    cudaFuncSetAttribute(newton_stage_list_kernel<N, G, RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    const int per_sm = RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB);
+    newton_stage_list_kernel<N, G, RED><<<(unsigned)(per_sm * (gv.nsm > 0 ? gv.nsm : 148)), NB, smem, s>>>(gv, a, cnt);
+    return 1;
+  }
   const long long blocks = (gv.nint + NB - 1) / NB;
-  const StageArgs a{Pn, PE, C, Gx, Pguess, dt_stage, max_iters, fresh, Piter, resnorm, status, iters};
-  newton_stage_kernel<N, G, RED><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
+  if (blocks == 0) return 0;
+  if (next_list) {
+    cudaFuncSetAttribute(newton_stage_kernel<N, G, RED, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    newton_stage_kernel<N, G, RED, true><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
+  } else {
+    cudaFuncSetAttribute(newton_stage_kernel<N, G, RED, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    newton_stage_kernel<N, G, RED, false><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt);
+  }
   return 1;
 }
 
 int launch_newton_stage(const GridView &gv, const double *Pn, const double *PE, const double *C, const double *G,
                         const double *Pguess, int fresh, double dt_stage, int max_iters, double *Piter, double *resnorm, int32_t *status,
-                        int32_t *iters, Counters *cnt, cudaStream_t s) {
+                        int32_t *iters, Counters *cnt, cudaStream_t s, const long long *list, long long nlist,
+                        long long *next_list) {
   const bool flat = (gv.metric == 0);
-#define GRIM_STAGE(NV, GG, RR) \
-  launch_stage_t<NV, GG, RR>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s)
+#define GRIM_STAGE(NV, GG, RR)                                                                                      \
+  launch_stage_t<NV, GG, RR>(gv, Pn, PE, C, G, Pguess, fresh, dt_stage, max_iters, Piter, resnorm, status, iters, cnt, s, \
+                             list, nlist, next_list)
   if (gv.reduced) {
     if (gv.nvar == 10) return flat ? GRIM_STAGE(10, GeomFlat, true) : GRIM_STAGE(10, GeomGen, true);
     return flat ? GRIM_STAGE(8, GeomFlat, true) : GRIM_STAGE(8, GeomGen, true);
