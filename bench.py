@@ -44,7 +44,7 @@ NCU_TRAFFIC_SOURCE = "profiles/r1g_ncu_full_stage_kernels.md"
 # upper figure.  Algorithmic fp64 work: DADD + DMUL + DFMA thread instructions of the same four kernels in the round's
 # first ncu capture (profiles/r1a_ncu_full_stage_kernels_baseline.md), frozen like the Newton count.
 ALG_BYTES_PER_ZONE_STAGE_FLUX = 400.0
-ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX = 4370.0
+ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX = 3997.0
 NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX = 1000.0
 FP64_INSTR_PER_CLK_PER_SM = 64.0                 # B200: 64 fp64 lanes per SM (guide: unit counts), 148 SMs
 N_SM = 148
@@ -297,13 +297,15 @@ def run_ours(args):
     # end to end through the C ABI with HOST buffers (pinned): H2D of P, one step, D2H of P, every step
     hP = torch.from_numpy(P0.copy()).pin_memory()
     e2e_steps = max(1, min(args.steps, 5))
-    slab.timestep_host(hP, dt)
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
+    e2e_s = float("nan")
+    if not args.no_e2e:
         slab.timestep_host(hP, dt)
-    barrier()
-    e2e_s = (time.perf_counter() - t0) / e2e_steps
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            slab.timestep_host(hP, dt)
+        barrier()
+        e2e_s = (time.perf_counter() - t0) / e2e_steps
 
     tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
     if world > 1:
@@ -404,6 +406,8 @@ def main():
     ap.add_argument("--flux-ct", action="store_true", help="flux-CT averaging of the B-field fluxes (not the headline)")
     ap.add_argument("--reduced", action="store_true",
                     help="the paper's reduced solve (B explicit, 7 x 7 Jacobian) instead of BASELINE's 10 unknowns")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs: keeps the launch list "
+                                                            "to the device-resident steps)")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads (config 2, Kerr step)")
     ap.add_argument("--dim", type=int, default=3, choices=[2, 3], help="2: the same generator on an n x n grid (X^2 slabs)")
     ap.add_argument("--backend", default="nccl", choices=["nccl", "gloo"],

@@ -223,6 +223,11 @@ int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t wide, int6
 /* End-to-end variants taking HOST buffers (pinned or pageable): copy in, run on the device, copy out, on the
  * context's stream; they return after the stream is synchronised.  Device staging buffers belong to the context.
  *   grim_timestep_host          : P_host N*Zg in/out; runs nsteps time steps (dt <= 0: chosen per step from cfl).
+ *                                 nsteps == 1 with dt > 0 on a 3-D grid of >= 64 X^3 planes (no flux-CT, no
+ *                                 GRIM_BC_NONE side): pipelined over slabs of X^3 planes -- copies of other slabs run
+ *                                 on two more streams while a slab's kernels run; same bits as grim_timestep.  In
+ *                                 that mode the ghost zones of P_host are neither read nor written (the boundary
+ *                                 conditions fill them on the device); otherwise the whole padded array is copied.
  *   grim_invert_primitives_host : U_host, P_host N*nz; iters/status/resnorm host outputs (may be NULL). */
 int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used);
 int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, double *P_host, int32_t *iters_host,

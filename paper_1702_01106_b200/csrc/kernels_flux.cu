@@ -801,12 +801,21 @@ speeds_kernel(const __grid_constant__ GridView gv, const double *__restrict__ cf
     }
     sp_loc[3] = ssum;
   }
+  // warp maxima -> block maxima in shared memory -> one atomic per figure and block
+  __shared__ double red[4][8];
 #pragma unroll
   for (int a = 0; a < 4; a++) {
     double v = sp_loc[a];
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    if ((threadIdx.x & 31) == 0 && v > 0.0) atomic_max_nonneg(&cnt->speeds[a], v);
+    if ((threadIdx.x & 31) == 0) red[a][threadIdx.x >> 5] = v;
+  }
+  __syncthreads();
+  if (threadIdx.x < 4) {
+    double v = red[threadIdx.x][0];
+#pragma unroll
+    for (int w = 1; w < 8; w++) v = fmax(v, red[threadIdx.x][w]);
+    if (v > 0.0) atomic_max_nonneg(&cnt->speeds[threadIdx.x], v);
   }
 }
 
