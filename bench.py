@@ -34,18 +34,19 @@ UNIT = "zone-updates/s"
 # instructions per zone and stage, compares included: profiles/r1g_ncu_full_stage_kernels.md.)
 ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 6114.0
 ALG_BYTES_PER_ZONE_STAGE_NEWTON = 8.0 * (10 + 10 + 10 + 10 + 3 + 10 + 1) + 4 * 4   # P^k,P_n,P_E,C,G in; P,|R| out; status,iters in/out
-# dram__bytes_read.sum + dram__bytes_write.sum of the Newton kernel per zone, mean of the stage-1 and stage-2 launches of
-# one ncu --set full capture (profiles/r1g_ncu_full_stage_kernels.md: 4.82 GB and 6.16 GB per 256^3 launch)
+# dram__bytes_read.sum + dram__bytes_write.sum of the Newton kernel per zone, mean of the stage-1 and stage-2 launches
+# (profiles/r2c_final_kernels.md: 288 B and 367 B per zone, ncu --set full captures of this round's final kernel)
 NCU_DRAM_BYTES_PER_ZONE_STAGE_NEWTON = 327.0
 NEWTON_KERNEL = "newton_stage_kernel<10,flat>"
-NCU_TRAFFIC_SOURCE = "profiles/r1g_ncu_full_stage_kernels.md"
+NCU_TRAFFIC_SOURCE = "profiles/r2c_final_kernels.md"
 # Flux class (3 face-flux launches + boundary-face boxes + stage constant) per zone and stage.  Algorithmic bytes: SURVEY
 # 8(d) "Flux + stage constant, EMHD": P_E 10 (x 1.3-1.5 halo re-read) + P_n 10 in, C 10 + G 3 out -> 320-400 B; the
 # upper figure.  Algorithmic fp64 work: DADD + DMUL + DFMA thread instructions of the same four kernels in the round's
-# first ncu capture (profiles/r1a_ncu_full_stage_kernels_baseline.md), frozen like the Newton count.
+# capture of the round-1 kernels (3997 per zone-stage: 3 x 1084 face + 744 stage constant; profiles/r2c_final_kernels.md
+# and r2b_optimisation_log.md), frozen like the Newton count.
 ALG_BYTES_PER_ZONE_STAGE_FLUX = 400.0
 ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX = 3997.0
-NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX = 1000.0
+NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX = 1075.0
 FP64_INSTR_PER_CLK_PER_SM = 64.0                 # B200: 64 fp64 lanes per SM (guide: unit counts), 148 SMs
 N_SM = 148
 
@@ -363,7 +364,7 @@ def run_ours(args):
             "bound": "hbm", "kernel": NEWTON_KERNEL, "achieved": hbm_ach,
             "peak": hbm_gbs, "unit": "GB/s", "frac": hbm_ach / hbm_gbs, "peak_source": which},
         "roofline_flux": None if not headline else {
-            "bound": "alu", "kernel": "face_flux_kernel x3 + stage_const (all flux-class launches of one stage)",
+            "bound": "alu", "kernel": "face_flux_tma_kernel x3 + face_box x3 + stage_const_tma_kernel (all flux-class launches of one stage)",
             "achieved": flux_alu, "peak": alu_peak, "unit": "T fp64 instr/s", "frac": flux_alu / alu_peak,
             "hbm_achieved_gbs": flux_hbm, "hbm_frac": flux_hbm / hbm_gbs,
             "traffic": NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX * zones, "traffic_source": NCU_TRAFFIC_SOURCE,
