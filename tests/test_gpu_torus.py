@@ -146,3 +146,31 @@ def test_config5_torus_256x256x128_one_step_every_zone():
 def test_config5_torus_small_50_steps():
     """Config 5's 50 steps (3-D torus with the phi-dependent noise) at 48 x 48 x 24, bit-identical throughout."""
     _run(48, 48, 24, 50, check_every=10)
+
+
+def test_sweep_policy_launch_counts():
+    """The stage solve runs in sweeps (first launch with kmax = 4, deferred zones by the list kernel: two Newton
+    launches per stage).  A run that never defers a zone (config 3: every zone takes 2 iterations) goes back to single
+    launches; the torus, which defers zones in every solve, stays in sweep mode.  Both modes give the oracle's bits (the
+    parity tests above and in test_gpu_parity.py run through whichever mode the policy picks)."""
+    import torch
+    from paper_1702_01106_b200 import workloads
+
+    def newton_launches_per_step(gk, P0, steps):
+        gc = cuda_grid(gk)
+        dP = to_dev(P0)
+        gc.fill_ghosts(dP)
+        dt, _ = gc.timestep(dP.clone(), 0.0, want_dt=True)
+        out = []
+        for _ in range(steps):
+            gc.set_timing(True)
+            gc.timestep(dP, dt)
+            torch.cuda.synchronize()
+            out.append(gc.get_timing()["newton"][1])
+            gc.set_timing(False)
+        return out
+
+    smooth = newton_launches_per_step(*workloads.config3(n=16), steps=12)
+    assert smooth[0] == 4 and smooth[-1] == 2, smooth            # sweeps at first, single launches once known quiet
+    torus = newton_launches_per_step(*workloads.fm_torus(48, 48, 1), steps=12)
+    assert all(n == 4 for n in torus), torus
