@@ -29,6 +29,12 @@ CASES = [
     ((19, 13, 11), 3, 10, og.MP5, 1.0),
     ((19, 13, 11), 3, 8, og.MINMOD, 2.0),
     ((150, 1, 1), 1, 10, og.MP5, 1.0),
+    # even padded X^1 extents: the TMA tile loads of the face-flux and stage-constant kernels (an odd extent, as in the
+    # cases above, takes the per-thread staging kernels); ragged tiles in every direction
+    ((38, 30, 1), 2, 8, og.MP5, 1.0),
+    ((34, 22, 1), 2, 10, og.MINMOD, 1.5),
+    ((20, 14, 12), 3, 10, og.MP5, 1.0),
+    ((130, 6, 5), 3, 8, og.MINMOD, 1.0),
 ]
 
 
