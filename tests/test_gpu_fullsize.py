@@ -57,9 +57,33 @@ def test_config3_fullsize_sampled(n):
                  bc=og.BC_NONE, nvar=10, recon=gk["recon"], limiter_theta=gk["limiter_theta"], gam=gk["gam"],
                  phi=gk["phi"], psi=gk["psi"], tau=gk["tau"], rtol=gk["rtol"], kmax=gk["kmax"], lsmax=gk["lsmax"])
     assert go.dx[0] == 1.0 / n
+    # per-zone iteration counts, statuses and residual norms of the first stage at full size (north star: "identical
+    # Newton iteration counts per zone"): grim_compute_fluxes + grim_newton_step on the whole grid, against the oracle's
+    # stage on each sampled sub-box -- every interior zone of a sub-box has its true stencil in stage 1
+    dP0 = to_dev(P0)
+    gc.fill_ghosts(dP0)
+    gc.compute_fluxes(dP0, dP0, 0.5 * dtu)
+    dPh = dP0.clone()
+    drn, dst, dit = gc.zeros(), gc.zeros(dtype=torch.int32), gc.zeros(dtype=torch.int32)
+    assert gc.newton_step(dP0, dP0, None, None, 0.5 * dtu, 0, dPh, drn, dst, dit) == 0
+    it_full = gc.interior(dit).cpu().numpy()
+    st_full = gc.interior(dst).cpu().numpy()
+    rn_full = gc.interior(drn).cpu().numpy()
+    del dP0, dPh, drn, dst, dit
+    hist_gpu, hist_ora = np.zeros(16, dtype=np.int64), np.zeros(16, dtype=np.int64)
     worst = 0.0
     for c in cs:
         Ps = subbox(P0, c, NG)
+        Cs, Gs, _ = go.stage_prepare(Ps, Ps, 0.5 * dtu)
+        Pq = Ps.copy()
+        _, (rno, sto, ito), _ = go.newton(Ps, Ps, Cs, Gs, 0.5 * dtu, Pq)
+        ii = [np.arange(c[a] - R, c[a] + R + 1) % n for a in range(3)]
+        sel = np.ix_(ii[0], ii[1], ii[2])
+        assert np.array_equal(it_full[sel], go.interior(ito)), c
+        assert np.array_equal(st_full[sel], go.interior(sto)), c
+        assert np.array_equal(rn_full[sel], go.interior(rno)), c
+        hist_gpu += np.bincount(it_full[sel].ravel(), minlength=16)[:16]
+        hist_ora += np.bincount(go.interior(ito).ravel(), minlength=16)[:16]
         so = go.timestep(Ps, dtu)
         got = P1[:, c[0], c[1], c[2]]
         exp = Ps[:, NG + R, NG + R, NG + R]
@@ -70,6 +94,7 @@ def test_config3_fullsize_sampled(n):
         gpu = P1[:, ii[0]][:, :, ii[1]][:, :, :, ii[2]]
         worst = max(worst, abs(gpu - blk).max())
     assert worst == 0.0
+    assert np.array_equal(hist_gpu, hist_ora) and hist_ora.sum() == len(cs) * (2 * R + 1) ** 3
 
 
 def test_config2_fullsize_sampled():
