@@ -268,7 +268,8 @@ def run_ours(args):
     zones = g.zones
     pbytes = dP.numel() * 8
     # the pipelined host path (1 GPU, 3-D) moves the interior X^3 planes only; the ghost planes are filled on the device
-    e2e_bytes = pbytes * g.n[2] // g.sz[2] if (world == 1 and args.dim == 3 and g.n[2] >= 64) else pbytes
+    pipelined = world == 1 and args.dim == 3 and g.n[2] >= 64 and zones >= 1500000
+    e2e_bytes = pbytes * g.n[2] // g.sz[2] if pipelined else pbytes
 
     def barrier():
         if world > 1:
@@ -349,7 +350,7 @@ def run_ours(args):
                 "d2h_bytes_per_step": e2e_bytes,
                 "how": "grim_timestep_host, pinned host buffer, one step per call: %s" % (
                     "interior X^3 planes copied slab by slab on two copy streams while the kernels of other slabs run"
-                    if world == 1 and args.dim == 3 else "copy in, step, copy out")},
+                    if pipelined else "copy in, step, copy out")},
         "gpu_launches": int(launches),
         "roofline": None if not headline else {
             "bound": "alu", "kernel": NEWTON_KERNEL, "achieved": alu_ach, "peak": alu_peak,

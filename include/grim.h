@@ -223,7 +223,7 @@ int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t wide, int6
 /* End-to-end variants taking HOST buffers (pinned or pageable): copy in, run on the device, copy out, on the
  * context's stream; they return after the stream is synchronised.  Device staging buffers belong to the context.
  *   grim_timestep_host          : P_host N*Zg in/out; runs nsteps time steps (dt <= 0: chosen per step from cfl).
- *                                 nsteps == 1 with dt > 0 on a 3-D grid of >= 64 X^3 planes (no flux-CT, no
+ *                                 nsteps == 1 with dt > 0 on a 3-D grid of >= 64 X^3 planes and >= 1.5 M zones (no flux-CT, no
  *                                 GRIM_BC_NONE side): pipelined over slabs of X^3 planes -- copies of other slabs run
  *                                 on two more streams while a slab's kernels run; same bits as grim_timestep.  In
  *                                 that mode the ghost zones of P_host are neither read nor written (the boundary

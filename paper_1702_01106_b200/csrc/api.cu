@@ -52,7 +52,7 @@ struct grim_ctx {
   double *invbuf;              // U, P, resnorm, iters, status of grim_invert_primitives_host
   long long invbuf_nz;
   int64_t launches;
-  int no_pipeline;             // GRIM_HOST_PIPELINE=0 in the environment: grim_timestep_host copies, steps, copies
+  int no_pipeline;             // GRIM_HOST_PIPELINE in the environment: 1 = "0" (never), -1 = "1" (always), 0 = unset
   // sweep policy of solve_stage: the deferred-zone counts of the recent sweep-mode solves arrive asynchronously in
   // pinned host memory; a run whose solves never defer a zone (smooth data) goes back to single launches and probes again
   // every GRIM_SWEEP_PROBE solves
@@ -219,8 +219,8 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   c->launches = 0;
   c->s_in = c->s_out = nullptr;
   {
-    const char *e = getenv("GRIM_HOST_PIPELINE");
-    c->no_pipeline = (e && e[0] == '0') ? 1 : 0;
+    const char *e = getenv("GRIM_HOST_PIPELINE");  // 0: never; 1: whenever the grid allows; unset: large grids only
+    c->no_pipeline = (e && e[0] == '0') ? 1 : (e && e[0] == '1') ? -1 : 0;
   }
   c->timing = 0;
   for (int k = 0; k < GRIM_NKCLASS; k++) { c->class_ms[k] = 0.0; c->class_n[k] = 0; }
@@ -790,8 +790,10 @@ extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, d
     for (int a = 0; a < 3; a++)
       for (int sd = 0; sd < 2; sd++)
         if (c->gv.ngd[a] > 0 && c->d.bc[a][sd] == GRIM_BC_NONE) caller_ghosts = true;
+    // slab-wise launches pay off from about 1.5 M zones (measured: 64^3 and 96^3 are faster copied whole)
+    const bool big = c->gv.nint >= 1500000 || c->no_pipeline < 0;
     if (nsteps == 1 && dt > 0.0 && c->gv.dim == 3 && c->gv.n[2] >= 4 * GRIM_HOST_SLABS && !c->gv.flux_ct && !caller_ghosts &&
-        !c->no_pipeline) {
+        big && c->no_pipeline <= 0) {
       rc = timestep_host_pipelined(c, P_host, dt);
       if (rc == GRIM_OK && dt_used) *dt_used = dt;
       return rc;

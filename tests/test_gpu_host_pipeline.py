@@ -11,8 +11,13 @@ pytestmark = pytest.mark.gpu
 
 
 def _check(gk, P0, steps=2):
+    import os
     import torch
-    gc = cuda_grid(gk)
+    os.environ["GRIM_HOST_PIPELINE"] = "1"       # small grids here: the library pipelines from 1.5 M zones on its own
+    try:
+        gc = cuda_grid(gk)
+    finally:
+        del os.environ["GRIM_HOST_PIPELINE"]
     dP = to_dev(P0)
     gc.fill_ghosts(dP)
     dt, _ = gc.timestep(dP.clone(), 0.0, want_dt=True)
