@@ -386,6 +386,22 @@ def test_minmod_with_two_ghost_zones(nvar, ct):
     assert np.array_equal(go.interior(Pc), go.interior(Po))
 
 
+def test_config3_48cubed_hundred_steps_in_place_branch():
+    """The same bar at 48^3 (110,592 zones, several blocks per SM in every kernel, ragged TMA tiles), through the branch
+    bench.py times (no statistics, P_{n+1} written in place) -- the sweep policy switches to single launches on the way
+    (the run never defers a zone) without a bit changing."""
+    import torch
+    from paper_1702_01106_b200 import workloads
+    gk, P0 = workloads.config3(n=48)
+    go, gc = oracle_grid(gk), cuda_grid(gk)
+    dt = go.choose_dt(P0)
+    Po, dP = P0.copy(), to_dev(P0)
+    for _ in range(100):
+        go.timestep(Po, dt)
+        gc.timestep(dP, dt)
+    assert np.array_equal(gc.interior(dP).cpu().numpy(), go.interior(Po))
+
+
 def test_config3_hundred_steps():
     """North star: max relative error per primitive <= 1e-8 after 100 steps, identical iteration counts.  Config 3's
     generator at 16^3, 100 steps: the result is bit-identical."""
