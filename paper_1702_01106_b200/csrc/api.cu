@@ -48,7 +48,8 @@ struct grim_ctx {
   long long list_cap;
   double *hostP;               // staging for the *_host entry points
   cudaStream_t s_in, s_out;    // copy streams of the pipelined grim_timestep_host
-  std::vector<cudaEvent_t> ev_in, ev_done;
+  cudaStream_t s_st2;          // its second compute stream (stage 2 of a slab beside stage 1 of a later one)
+  std::vector<cudaEvent_t> ev_in, ev_done, ev_s1;
   double *invbuf;              // U, P, resnorm, iters, status of grim_invert_primitives_host
   long long invbuf_nz;
   int64_t launches;
@@ -70,15 +71,16 @@ struct grim_ctx {
 
 // records an event pair around the launches enqueued by `body` when timing is on
 template <class F>
-static int timed(grim_ctx *c, int kclass, F body) {
+static int timed(grim_ctx *c, int kclass, F body, cudaStream_t on = nullptr) {
   if (!c->timing) return body();
+  if (!on) on = c->stream;
   KernelSpan sp;
   sp.kclass = kclass;
   cudaEventCreate(&sp.e0);
   cudaEventCreate(&sp.e1);
-  cudaEventRecord(sp.e0, c->stream);
+  cudaEventRecord(sp.e0, on);
   int n = body();
-  cudaEventRecord(sp.e1, c->stream);
+  cudaEventRecord(sp.e1, on);
   sp.launches = n;
   c->spans.push_back(sp);
   return n;
@@ -166,6 +168,8 @@ extern "C" void grim_free(grim_ctx *c) {
     if (p) cudaFree(p);
   for (auto e : c->ev_in) cudaEventDestroy(e);
   for (auto e : c->ev_done) cudaEventDestroy(e);
+  for (auto e : c->ev_s1) cudaEventDestroy(e);
+  if (c->s_st2) cudaStreamDestroy(c->s_st2);
   if (c->sweep_counts) {
     cudaFreeHost(c->sweep_counts);
     for (int q = 0; q < 4; q++) cudaEventDestroy(c->sweep_ev[q]);
@@ -217,7 +221,7 @@ extern "C" int grim_init_grid(grim_ctx **out, const grim_grid_desc *d) {
   c->stream = (cudaStream_t)d->stream;
   c->metric_set = 0;
   c->launches = 0;
-  c->s_in = c->s_out = nullptr;
+  c->s_in = c->s_out = c->s_st2 = nullptr;
   {
     const char *e = getenv("GRIM_HOST_PIPELINE");  // 0: never; 1: whenever the grid allows; unset: large grids only
     c->no_pipeline = (e && e[0] == '0') ? 1 : (e && e[0] == '1') ? -1 : 0;
@@ -695,6 +699,9 @@ extern "C" int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t
 #ifndef GRIM_HOST_SLABS
 #define GRIM_HOST_SLABS 16
 #endif
+#ifndef GRIM_HOST_EDGE
+#define GRIM_HOST_EDGE 4
+#endif
 static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
   const GridView &gv = c->gv;
   cudaStream_t s = c->stream;
@@ -702,21 +709,40 @@ static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
   const size_t plane = (size_t)gv.sz[0] * gv.sz[1], pitch = (size_t)gv.zg * 8;
   if (!c->s_in) CU(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
   if (!c->s_out) CU(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
+  if (!c->s_st2) CU(cudaStreamCreateWithFlags(&c->s_st2, cudaStreamNonBlocking));
   while ((int)c->ev_in.size() < K + 1) {
     cudaEvent_t e;
     CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     c->ev_in.push_back(e);
     CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
     c->ev_done.push_back(e);
+    CU(cudaEventCreateWithFlags(&e, cudaEventDisableTiming));
+    c->ev_s1.push_back(e);
   }
+  cudaStream_t s2 = c->s_st2;
   int k0[GRIM_HOST_SLABS + 1];
-  for (int q = 0; q <= K; q++) k0[q] = (int)((long long)n3 * q / K / 4 * 4);  // multiples of the 4-plane flux tiles
-  k0[K] = n3;
+  // Slab boundaries, multiples of the 4-plane flux tiles.  The first and the last slab are coupled through the X^3
+  // boundary: they arrive first and finish last, nothing overlaps their copies -- so they are thin (GRIM_HOST_EDGE
+  // planes) and the K - 2 slabs between them share the rest.
+  {
+    const int e = (n3 >= 16 * GRIM_HOST_EDGE) ? GRIM_HOST_EDGE : 0;
+    if (e) {
+      k0[0] = 0;
+      k0[1] = e;
+      for (int q = 2; q < K - 1; q++) k0[q] = e + (int)((long long)(n3 - 2 * e) * (q - 1) / (K - 2) / 4 * 4);
+      k0[K - 1] = n3 - e;
+      k0[K] = n3;
+    } else {
+      for (int q = 0; q <= K; q++) k0[q] = (int)((long long)n3 * q / K / 4 * 4);
+      k0[K] = n3;
+    }
+  }
   double *d = c->hostP;
   // the copy streams start after whatever the caller enqueued on the context's stream
   CU(cudaEventRecord(c->ev_in[K], s));
   CU(cudaStreamWaitEvent(c->s_in, c->ev_in[K], 0));
   CU(cudaStreamWaitEvent(c->s_out, c->ev_in[K], 0));
+  CU(cudaStreamWaitEvent(s2, c->ev_in[K], 0));
   auto h2d = [&](int q) {
     const size_t off = (size_t)(ng + k0[q]) * plane;
     cudaMemcpy2DAsync(d + off, pitch, P_host + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
@@ -744,11 +770,16 @@ static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
     c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(g, d, d, dt1, c->C, c->G, c->Fface, c->cface, nullptr, s); });
     c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(g, d, d, c->C, c->G, d, 1, dt1, 0, c->Ph, c->resnorm, c->status, c->iters, c->cnt, s); });
   };
-  auto stage2 = [&](int q) {
+  // Stage 2 runs on a second stream: stage 2 of slab q needs stage 1 of slabs q - 1, q, q + 1 (event ev_s1[q + 1]) and
+  // is independent of stage 1 of the later slabs, which the first stream goes on with -- the two streams' kernels touch
+  // disjoint plane ranges of every scratch array (slab q against slabs >= q + 2), and the ramps and tails of the small
+  // slab-wise launches overlap instead of adding up.
+  auto stage2 = [&](int q, cudaEvent_t after) {
     const GridView g = slab(q);
-    c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(g, c->Ph, d, dt, c->C, c->G, c->Fface, c->cface, nullptr, s); });
-    c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(g, d, c->Ph, c->C, c->G, c->Ph, 1, dt, 0, d, c->resnorm, c->status, c->iters, c->cnt, s); });
-    cudaEventRecord(c->ev_done[q], s);
+    cudaStreamWaitEvent(s2, after, 0);
+    c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(g, c->Ph, d, dt, c->C, c->G, c->Fface, c->cface, nullptr, s2); }, s2);
+    c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(g, d, c->Ph, c->C, c->G, c->Ph, 1, dt, 0, d, c->resnorm, c->status, c->iters, c->cnt, s2); }, s2);
+    cudaEventRecord(c->ev_done[q], s2);
     cudaStreamWaitEvent(c->s_out, c->ev_done[q], 0);
     const size_t off = (size_t)(ng + k0[q]) * plane;
     cudaMemcpy2DAsync(P_host + off, pitch, d + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
@@ -767,13 +798,16 @@ static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
     }
     stage1(q);
     ghosts01(c->Ph, q);
-    if (q >= 2) stage2(q - 1);
+    CU(cudaEventRecord(c->ev_s1[q], s));
+    if (q >= 2) stage2(q - 1, c->ev_s1[q]);
   }
   ghosts2(c->Ph);
-  stage2(K - 1);
-  stage2(0);
+  CU(cudaEventRecord(c->ev_s1[K], s));
+  stage2(K - 1, c->ev_s1[K]);
+  stage2(0, c->ev_s1[K]);
   int rc = check_launch(c, "pipelined timestep");
   CU(cudaStreamSynchronize(c->s_out));
+  CU(cudaStreamSynchronize(s2));
   CU(cudaStreamSynchronize(s));
   return rc;
 }
