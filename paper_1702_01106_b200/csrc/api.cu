@@ -422,7 +422,12 @@ static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const 
                        int32_t *status, int32_t *iters) {
   cudaStream_t s = c->stream;
   bool sweeps = GRIM_STAGE_SWEEP > 0 && gv.sp.kmax > GRIM_STAGE_SWEEP;
-  if (sweeps) {
+  // While the stream is being captured into a CUDA graph the policy below (event queries, a pinned read-back) must not
+  // run: a captured step always takes the two-launch form, whose list length stays on the device.
+  cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
+  cudaStreamIsCapturing(s, &cap);
+  const bool capturing = cap != cudaStreamCaptureStatusNone;
+  if (sweeps && !capturing) {
     // Both modes give the same results zone for zone; the policy only decides which is faster.  Collect the counts of
     // earlier sweep-mode solves that have landed: 4 in a row without a deferred zone -> single launches for a while.
     if (!c->sweep_counts) {
@@ -467,7 +472,7 @@ static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const 
   if (rc || !sweeps) return rc;
   // the second sweep reads the list length from the device: no synchronisation; the length also goes to the host,
   // asynchronously, for the sweep policy
-  {
+  if (!capturing) {
     const int q = c->sweep_slot;
     if (!c->sweep_pending[q]) {
       CU(cudaMemcpyAsync(&c->sweep_counts[q], &c->cnt->list_count, sizeof(unsigned long long), cudaMemcpyDeviceToHost, s));
