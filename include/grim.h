@@ -170,7 +170,10 @@ int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_target, cons
  * Ghost zones of P_inout on return are those the first ghost fill gave P_n (every call refills them; ghosts of a
  * GRIM_BC_NONE side are the caller's and are used unchanged for both stages).
  *   dt <= 0: dt = cfl / max_z sum_d c^d/dX^d (C-15).   dt_used : host or NULL.   stats : host or NULL
- * (requesting dt_used or stats synchronises the stream). */
+ * (requesting dt_used or stats synchronises the stream). 
+ * With dt > 0, dt_used == NULL and stats == NULL the call only enqueues work on the context's stream (no
+ * synchronisation, no allocation once the context has run a step): it may be captured into a CUDA graph on that
+ * stream and replayed (tests/test_gpu_host_pipeline.py). */
 int grim_timestep(grim_ctx *c, double *P_inout, double dt, double *dt_used, grim_step_stats *stats);
 
 /* ---- helpers beyond the six ------------------------------------------------------------------------------ */
