@@ -253,7 +253,10 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         if args.backend == "nccl":
-            os.environ.setdefault("NCCL_DEBUG", "WARN")
+            # the communicator log (rank count, transports, NVLS) goes to a file: stdout carries the one JSON line
+            os.environ.setdefault("NCCL_DEBUG", "INFO")
+            os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
+            os.environ.setdefault("NCCL_DEBUG_FILE", os.path.join(tempfile.gettempdir(), "grim_bench_nccl_%h_%p.log"))
             dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         else:
             dist.init_process_group("gloo")
@@ -344,7 +347,8 @@ def run_ours(args):
                    "update": "one zone advanced one grim_timestep = 2 stages x (ghosts, MP5+LLF fluxes, stage "
                              "constants, fused Newton solve)", "dt": "fixed: CFL 0.5 on the initial data",
                    "l2": "inputs (%.2f GB per field) larger than L2" % (pbytes / 1e9),
-                   "parallelism": "slab%d" % world, "backend": args.backend if world > 1 else None},
+                   "parallelism": "slab%d" % world, "backend": args.backend if world > 1 else None,
+                   "nccl_log": os.environ.get("NCCL_DEBUG_FILE") if (world > 1 and args.backend == "nccl") else None},
         "clocks": clocks,
         "e2e": {"value": zones * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": e2e_bytes,
                 "d2h_bytes_per_step": e2e_bytes,
