@@ -231,6 +231,8 @@ int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t wide, int6
  *                                 on two more streams while a slab's kernels run; same bits as grim_timestep.  In
  *                                 that mode the ghost zones of P_host are neither read nor written (the boundary
  *                                 conditions fill them on the device); otherwise the whole padded array is copied.
+ *                                 Environment GRIM_HOST_PIPELINE=0 / 1 (read at grim_init_grid): never / whenever the
+ *                                 grid allows it, regardless of size.
  *   grim_invert_primitives_host : U_host, P_host N*nz; iters/status/resnorm host outputs (may be NULL). */
 int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used);
 int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, double *P_host, int32_t *iters_host,
