@@ -271,7 +271,7 @@ def run_ours(args):
     zones = g.zones
     pbytes = dP.numel() * 8
     # the pipelined host path (1 GPU, 3-D) moves the interior X^3 planes only; the ghost planes are filled on the device
-    pipelined = world == 1 and args.dim == 3 and g.n[2] >= 64 and zones >= 1500000
+    pipelined = world == 1 and args.dim == 3 and g.n[2] >= 64 and zones >= 1500000 and not args.flux_ct
     e2e_bytes = pbytes * g.n[2] // g.sz[2] if pipelined else pbytes
 
     def barrier():
