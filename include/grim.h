@@ -179,7 +179,8 @@ int grim_timestep(grim_ctx *c, double *P_inout, double dt, double *dt_used, grim
 /* ---- helpers beyond the six ------------------------------------------------------------------------------ */
 
 void grim_free(grim_ctx *c);
-const char *grim_last_error(const grim_ctx *c); /* NULL ctx: error of the last failed grim_init_grid */
+const char *grim_last_error(const grim_ctx *c); /* NULL ctx: error of the last failed grim_init_grid or
+                                                    grim_invert_primitives_static */
 int grim_version(void);
 
 /* Padded zone count Zg and padded extents (host out, may be NULL). */
@@ -237,6 +238,45 @@ int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t wide, int6
 int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used);
 int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, double *P_host, int32_t *iters_host,
                                 int32_t *status_host, double *resnorm_host);
+
+/* ---- for callers that must not allocate device memory -------------------------------------------------------
+ *
+ * Every call above needs a grim_ctx, and grim_init_grid buys the context's scratch with cudaMalloc (so do
+ * grim_invert_primitives and the *_host variants when their lists or staging buffers grow).  Some users of this
+ * library cannot do that: a plug-in of a host application (a simulation code, a PyTorch process) whose own memory pool
+ * has already claimed the device's memory at start-up, so that a cudaMalloc from a library either fails or takes
+ * memory the pool has promised elsewhere; and a caller inside a time-critical loop, because cudaMalloc and cudaFree
+ * wait for the whole device and stall the application's other streams.  Such a caller owns device buffers for its
+ * inputs and outputs (carved from its pool) but can give the library nothing else.
+ *
+ * grim_invert_primitives_static is grim_invert_primitives (O-10, BASELINE config 2; same kernels' arithmetic, same
+ * result bit for bit, zone for zone) for them: it takes no context and calls no cudaMalloc, cudaFree or any other
+ * allocating routine, in any call, the first included.  The two active-zone lists and the counters that the sweeps
+ * need live in a fixed array inside the library's device image (a file-scope `static __device__` array in
+ * kernels_newton.cu) of 256 + 8 * GRIM_STATIC_MAX_ZONES bytes = 8 MiB + 256 B.  Every GPU on which this library is
+ * loaded holds that array from the moment the CUDA module loads until the process exits, whether or not this entry
+ * point is ever called.
+ *
+ *   d  : HOST.  Read: model, gamma, phi, psi, closure, tau, fd_eps, eps_bt, rtol, kmax, lsmax (validated as in
+ *        grim_init_grid), device, stream.  The grid fields (n1.., ng, dim, extents, bc, recon, ...) are ignored.
+ *   nz : zones, 0 <= nz <= GRIM_STATIC_MAX_ZONES; a larger nz is refused with GRIM_EINVAL and a message that states
+ *        the limit (split the batch, or use grim_invert_primitives).  nz == 0 returns GRIM_OK and does nothing.
+ *   U_target, geom, P_inout, iters, status, resnorm : DEVICE, the caller's, exactly as for grim_invert_primitives.
+ *
+ * Behaviour the caller must know:
+ *   - The first call on each device looks up the device address of the array (cudaGetSymbolAddress) and raises the
+ *     kernels' shared-memory limit, once, and remembers both per device.  Make that first call during set-up, before
+ *     starting any stream capture on that device.
+ *   - All calls in the process share the one array per device, and it keeps whatever the previous call left in it.  The
+ *     entry point zeroes its counters itself before every sweep; the lists need no clearing (only the entries a sweep
+ *     has just written are read).  Because the array is shared, two calls whose kernels overlap on the same GPU
+ *     (different streams, or different host threads) race on it and corrupt each other's lists: serialise them.
+ *   - d->device becomes the calling thread's current device.  The call enqueues on d->stream and returns after
+ *     synchronising it (each sweep reads the number of zones still iterating back to the host).
+ *   - Errors: GRIM_EINVAL / GRIM_ECUDA as elsewhere; the text is at grim_last_error(NULL).  No CPU fallback. */
+#define GRIM_STATIC_MAX_ZONES (1 << 20)
+int grim_invert_primitives_static(const grim_grid_desc *d, int64_t nz, const double *U_target, const double *geom,
+                                  double *P_inout, int32_t *iters, int32_t *status, double *resnorm);
 
 /* Number of kernels the library has launched on this context since creation (host bookkeeping). */
 int64_t grim_launch_count(const grim_ctx *c);

@@ -63,6 +63,7 @@ _SIGNATURES = {
     "grim_arith_selftest": (C.c_int, [_vp, _i64, _i64, _i32, _pi64]),
     "grim_timestep_host": (C.c_int, [_vp, _vp, _i32, _dbl, _pd]),
     "grim_invert_primitives_host": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp]),
+    "grim_invert_primitives_static": (C.c_int, [C.POINTER(GridDesc), _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
     "grim_launch_count": (_i64, [_vp]),
     "grim_set_timing": (C.c_int, [_vp, _i32]),
     "grim_get_timing": (C.c_int, [_vp, _pd, _pi64]),
@@ -120,6 +121,46 @@ def _host_ptr(t, dtype=None):
     if dtype is not None and t.dtype != dtype:
         raise GrimError("expected dtype %s, got %s" % (dtype, t.dtype))
     return C.c_void_p(t.data_ptr())
+
+
+STATIC_MAX_ZONES = 1 << 20   # GRIM_STATIC_MAX_ZONES of include/grim.h
+
+
+def invert_primitives_static(U_target, P_inout, iters, status, resnorm, geom=None, model=IDEAL, gamma=4.0 / 3.0,
+                             phi=1.0, psi=1.0, closure=0, tau=1.0, fd_eps=4e-8, eps_bt=1e-4, rtol=1e-14, kmax=8,
+                             lsmax=5, device=0, stream=None):
+    """grim_invert_primitives_static: the standalone inversion for a caller that must not allocate device memory.
+
+    A `Grid` cannot be used by code that runs inside an application whose memory pool already holds the device's
+    memory, or inside a loop that cannot afford the device-wide stall of cudaMalloc/cudaFree: creating a `Grid`
+    allocates its scratch, and `Grid.invert_primitives` allocates its zone lists.  This function needs no `Grid` and
+    allocates nothing, on any call: its scratch is a fixed 8 MiB array inside the library's device image, which is why
+    at most STATIC_MAX_ZONES (2^20) zones fit in one call (more raises GrimError) and why two calls must never run on
+    the same GPU at the same time (they would share, and corrupt, that array).  Make the first call on a device during
+    set-up: that call looks up the array's device address.  Arguments and results are those of
+    `Grid.invert_primitives`, bit for bit; the model and solver parameters are passed here instead of coming from a
+    grid.  Returns after the stream is synchronised."""
+    import torch
+    d = GridDesc()
+    d.n1 = d.n2 = d.n3 = 1
+    d.dim = 1
+    d.model, d.gamma, d.phi, d.psi, d.closure = model, gamma, phi, psi, closure
+    d.tau_mode, d.tau = TAU_CONST, tau
+    d.fd_eps, d.eps_bt, d.atol, d.rtol, d.kmax, d.lsmax = fd_eps, eps_bt, 0.0, rtol, kmax, lsmax
+    d.device = device
+    if stream is None:
+        stream = torch.cuda.current_stream(device).cuda_stream
+    d.stream = stream
+    nz = P_inout.shape[1]
+    if geom is not None and tuple(geom.shape) != (15, nz):
+        raise GrimError("invert_primitives_static: geom must have shape (15, %d)" % nz)
+    L = lib()
+    f64, i32 = torch.float64, torch.int32
+    rc = L.grim_invert_primitives_static(C.byref(d), nz, _ptr(U_target, f64), _ptr(geom, f64), _ptr(P_inout, f64),
+                                         _ptr(iters, i32), _ptr(status, i32), _ptr(resnorm, f64))
+    if rc != 0:
+        msg = L.grim_last_error(None)
+        raise GrimError("grim_invert_primitives_static failed (%d): %s" % (rc, msg.decode() if msg else ""))
 
 
 class Grid:

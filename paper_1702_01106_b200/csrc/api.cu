@@ -102,6 +102,11 @@ static void drain_spans(grim_ctx *c) {
 
 static std::string g_init_error;
 
+// the context-free entry point (kernels_newton.cu) reports through grim_last_error(NULL) too
+namespace grim {
+void set_global_error(const char *msg) { g_init_error = msg ? msg : ""; }
+}  // namespace grim
+
 static int fail(grim_ctx *c, int code, const std::string &msg) {
   if (c) c->err = msg;
   else g_init_error = msg;

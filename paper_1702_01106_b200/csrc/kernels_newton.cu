@@ -359,3 +359,202 @@ int launch_prim_to_conserved(const GridView &gv, long long nz, const double *P, 
 }
 
 }  // namespace grim
+
+// ---------------------------------------------------------------------------------------------------------
+// grim_invert_primitives_static (include/grim.h): the standalone inversion for callers that cannot allocate
+// device memory -- plug-ins of an application whose memory pool already owns the device, and time-critical
+// loops that cannot afford the device-wide wait of cudaMalloc / cudaFree.  It needs no grim_ctx (whose
+// creation allocates) and allocates nothing itself.  The scratch of the sweeps -- the counters and the two
+// lists of zones that are still iterating -- is the array below: part of the library's device image, so
+// every GPU that loads the library carries its 8 MiB + 256 B until the process ends.
+//
+// Everything that touches the array is in this file.  Device code may name `static_scratch` directly.  HOST
+// code may not: on the host the name is only a handle for the runtime (a kernel handed `static_scratch` from
+// host code would fault, or on a system where the GPU can read host memory, quietly use the wrong bytes).
+// The host gets the real device address once per device from cudaGetSymbolAddress, with that device current,
+// and passes it to the kernels and to cudaMemsetAsync.
+//
+// Layout: [0, 56)  Counters      [256, 256 + 4 MAXZ)  list 0      [256 + 4 MAXZ, 256 + 8 MAXZ)  list 1
+// (zone numbers fit 32 bits because nz <= GRIM_STATIC_MAX_ZONES).  The array is shared by every call on the
+// device and keeps the previous call's contents; see the header for what that means for the caller.
+// ---------------------------------------------------------------------------------------------------------
+#include <string.h>
+
+#include <mutex>
+#include <string>
+
+#include "../../include/grim.h"
+
+namespace grim {
+
+static constexpr long long STATIC_MAXZ = GRIM_STATIC_MAX_ZONES;
+static constexpr size_t STATIC_LIST_OFFSET = 256;
+static constexpr size_t STATIC_SCRATCH_BYTES = STATIC_LIST_OFFSET + 2 * sizeof(uint32_t) * (size_t)STATIC_MAXZ;
+static_assert(sizeof(Counters) <= STATIC_LIST_OFFSET, "counters must fit in front of the lists");
+
+static __device__ __align__(256) unsigned char static_scratch[STATIC_SCRATCH_BYTES];
+
+// invert_kernel with 32-bit lists at caller-supplied addresses (the host passes addresses inside static_scratch).
+// Zones are solved by the same invert_zone as the allocating path, so a zone's result is the same bits.
+template <int N, class G>
+__global__ void __launch_bounds__(NB, N == 8 ? GRIM_N8_MINB : 256 / NB)
+invert_static_kernel(const __grid_constant__ GridView gv, const __grid_constant__ InvertArgs a, Counters *cnt,
+                     const uint32_t *__restrict__ list, uint32_t *__restrict__ next_list) {
+  extern __shared__ double smem[];
+  const long long t = (long long)blockIdx.x * NB + threadIdx.x;
+  int res = 0;
+  long long z = -1;
+  if (t < a.nlist) {
+    z = a.first ? t : (long long)list[t];
+    SpecArith ar;
+    res = invert_zone<N, G>(ar, gv, a, z, smem + threadIdx.x);
+    if (res < 0) res = invert_zone_replay<N, G>(gv, a, z, smem + threadIdx.x);
+  }
+  const int active_after = res & 1;
+  const unsigned ballot = __ballot_sync(0xffffffffu, active_after);
+  const int lane = threadIdx.x & 31;
+  unsigned long long base = 0;
+  if (lane == 0 && ballot) base = atomicAdd(&cnt->list_count, (unsigned long long)__popc(ballot));
+  base = __shfl_sync(0xffffffffu, base, 0);
+  if (active_after) next_list[base + __popc(ballot & ((1u << lane) - 1u))] = (uint32_t)z;
+  unsigned long long b = __reduce_add_sync(0xffffffffu, (unsigned)(res >> 1));
+  if (lane == 0 && b) atomicAdd(&cnt->backtracks, b);
+}
+
+template <int N, class G>
+static cudaError_t static_kernel_setup() {
+  return cudaFuncSetAttribute(invert_static_kernel<N, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)((size_t)(N * N + N) * NB * sizeof(double)));
+}
+
+template <int N, class G>
+static void static_kernel_launch(const GridView &gv, const InvertArgs &a, Counters *cnt, const uint32_t *list,
+                                 uint32_t *next_list, cudaStream_t s) {
+  const size_t smem = (size_t)(N * N + N) * NB * sizeof(double);
+  const long long blocks = (a.nlist + NB - 1) / NB;
+  invert_static_kernel<N, G><<<(unsigned)blocks, NB, smem, s>>>(gv, a, cnt, list, next_list);
+}
+
+// Device address of static_scratch on `device` (which must be current); the first call per device asks the runtime
+// and configures the four kernel variants.  Returns cudaSuccess or the failing call's code.
+static constexpr int STATIC_MAX_DEVICES = 64;
+static std::mutex static_mu;
+static unsigned char *static_addr[STATIC_MAX_DEVICES];
+
+static cudaError_t static_scratch_address(int device, unsigned char **out) {
+  std::lock_guard<std::mutex> lock(static_mu);
+  if (!static_addr[device]) {
+    int major = 0;
+    cudaError_t e = cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device);
+    if (e != cudaSuccess) return e;
+    if (major != 10) return cudaErrorNoKernelImageForDevice;  // sm_100a only, as grim_init_grid
+    unsigned char *p = nullptr;
+    e = cudaGetSymbolAddress((void **)&p, static_scratch);
+    if (e != cudaSuccess) return e;
+    if (!p) return cudaErrorInvalidSymbol;
+    if ((e = static_kernel_setup<8, GeomFlat>()) != cudaSuccess) return e;
+    if ((e = static_kernel_setup<8, GeomGen>()) != cudaSuccess) return e;
+    if ((e = static_kernel_setup<10, GeomFlat>()) != cudaSuccess) return e;
+    if ((e = static_kernel_setup<10, GeomGen>()) != cudaSuccess) return e;
+    static_addr[device] = p;
+  }
+  *out = static_addr[device];
+  return cudaSuccess;
+}
+
+void set_global_error(const char *msg);  // api.cu: the text grim_last_error(NULL) returns
+
+static int static_fail(int code, const std::string &msg) {
+  set_global_error(msg.c_str());
+  return code;
+}
+
+}  // namespace grim
+
+extern "C" int grim_invert_primitives_static(const grim_grid_desc *d, int64_t nz, const double *U_target,
+                                             const double *geom, double *P_inout, int32_t *iters, int32_t *status,
+                                             double *resnorm) {
+  using namespace grim;
+  const char *me = "grim_invert_primitives_static: ";
+  if (!d) return static_fail(GRIM_EINVAL, std::string(me) + "null descriptor");
+  if (nz < 0 || (nz > 0 && (!U_target || !P_inout || !iters || !status || !resnorm)))
+    return static_fail(GRIM_EINVAL, std::string(me) + "bad argument");
+  if (nz > STATIC_MAXZ)
+    return static_fail(GRIM_EINVAL, std::string(me) + "nz = " + std::to_string((long long)nz) +
+                                        " exceeds GRIM_STATIC_MAX_ZONES = " + std::to_string(STATIC_MAXZ) +
+                                        " (the fixed scratch array holds no more): split the batch or use "
+                                        "grim_invert_primitives");
+  if (d->model != GRIM_IDEAL && d->model != GRIM_EMHD) return static_fail(GRIM_EINVAL, std::string(me) + "model must be 8 or 10");
+  if (!(d->gamma > 1.0)) return static_fail(GRIM_EINVAL, std::string(me) + "adiabatic index must exceed 1");
+  if (!(d->fd_eps > 0.0) || d->kmax < 0 || d->lsmax < 0) return static_fail(GRIM_EINVAL, std::string(me) + "bad solver parameters");
+  if (d->closure != GRIM_CLOSURE_CS2TAU && d->closure != GRIM_CLOSURE_CONST)
+    return static_fail(GRIM_EINVAL, std::string(me) + "unknown closure");
+  if (d->model == GRIM_EMHD && !(d->tau_mode == GRIM_TAU_R32 || d->tau > 0.0))
+    return static_fail(GRIM_EINVAL, std::string(me) + "tau_R must be positive");
+  if (nz == 0) return GRIM_OK;
+
+#define SCU(call)                                                                                       \
+  do {                                                                                                  \
+    cudaError_t e_ = (call);                                                                            \
+    if (e_ != cudaSuccess) return static_fail(GRIM_ECUDA, std::string(me) + #call + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0)
+    return static_fail(GRIM_ECUDA, std::string(me) + "no CUDA device: this library has no CPU fallback");
+  if (d->device < 0 || d->device >= ndev || d->device >= STATIC_MAX_DEVICES)
+    return static_fail(GRIM_EINVAL, std::string(me) + "device ordinal out of range");
+  SCU(cudaSetDevice(d->device));
+  unsigned char *base = nullptr;
+  SCU(static_scratch_address(d->device, &base));
+  Counters *cnt = (Counters *)base;
+  uint32_t *lists[2] = {(uint32_t *)(base + STATIC_LIST_OFFSET),
+                        (uint32_t *)(base + STATIC_LIST_OFFSET + sizeof(uint32_t) * (size_t)STATIC_MAXZ)};
+  cudaStream_t s = (cudaStream_t)d->stream;
+
+  // the part of the grid view the inversion reads: model, solver parameters, constant tau_R
+  GridView gv;
+  memset(&gv, 0, sizeof(gv));
+  gv.nvar = d->model;
+  gv.m.gam = d->gamma;
+  gv.m.gm1 = d->gamma - 1.0;
+  gv.m.phi = d->phi;
+  gv.m.psi = d->psi;
+  gv.m.closure = d->closure ? 1 : 0;
+  gv.tau_const = d->tau;
+  gv.sp.fd_eps = d->fd_eps;
+  gv.sp.eps_bt = d->eps_bt;
+  gv.sp.atol = d->atol;
+  gv.sp.rtol = d->rtol;
+  gv.sp.kmax = d->kmax;
+  gv.sp.lsmax = d->lsmax;
+
+  // Sweeps of 4 iterations over the zones that are still iterating, as grim_invert_primitives runs them (where a
+  // zone's iteration pauses does not change its result).  The counters start every sweep at zero; the list a sweep
+  // reads was written in full by the sweep before it, so stale entries of earlier calls are never read.
+  const int sweep = 4;
+  long long nlist = nz;
+  int first = 1, cur = 0, done_iters = 0;
+  while (nlist > 0) {
+    SCU(cudaMemsetAsync(cnt, 0, sizeof(Counters), s));
+    const InvertArgs a{nz, nlist, nullptr, U_target, P_inout, iters, status, resnorm, sweep, first, nullptr, geom};
+    if (gv.nvar == 10) {
+      if (geom) static_kernel_launch<10, GeomGen>(gv, a, cnt, lists[cur], lists[cur ^ 1], s);
+      else static_kernel_launch<10, GeomFlat>(gv, a, cnt, lists[cur], lists[cur ^ 1], s);
+    } else {
+      if (geom) static_kernel_launch<8, GeomGen>(gv, a, cnt, lists[cur], lists[cur ^ 1], s);
+      else static_kernel_launch<8, GeomFlat>(gv, a, cnt, lists[cur], lists[cur ^ 1], s);
+    }
+    SCU(cudaGetLastError());
+    unsigned long long left = 0;
+    SCU(cudaMemcpyAsync(&left, &cnt->list_count, sizeof(left), cudaMemcpyDeviceToHost, s));
+    SCU(cudaStreamSynchronize(s));
+    nlist = (long long)left;
+    cur ^= 1;
+    first = 0;
+    done_iters += sweep;
+    if (done_iters > d->kmax + 8) break;  // cannot happen: every zone reaches kmax
+  }
+#undef SCU
+  return GRIM_OK;
+}
