@@ -37,6 +37,10 @@ ALG_BYTES_PER_ZONE_STAGE_NEWTON = 8.0 * (10 + 10 + 10 + 10 + 3 + 10 + 1) + 4 * 4
 # dram__bytes_read.sum + dram__bytes_write.sum of the Newton kernel per zone, mean of the stage-1 and stage-2 launches
 # (profiles/r2c_final_kernels.md: 288 B and 367 B per zone, ncu --set full captures of this round's final kernel)
 NCU_DRAM_BYTES_PER_ZONE_STAGE_NEWTON = 327.0
+# What the current kernel executes (DADD + DMUL + DFMA per zone and stage at 2 iterations, profiles/r2c_final_kernels.md):
+# fewer than the frozen algorithmic count, because structural zeros of the Jacobian and of the LU are skipped.
+# roofline.frac credits the frozen count (work the method defines); roofline.frac_executed is the fp64-pipe utilisation.
+EXECUTED_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 5274.0
 NEWTON_KERNEL = "newton_stage_kernel<10,flat>"
 NCU_TRAFFIC_SOURCE = "profiles/r2c_final_kernels.md"
 # Flux class (3 face-flux launches + boundary-face boxes + stage constant) per zone and stage.  Algorithmic bytes: SURVEY
@@ -253,10 +257,10 @@ def run_ours(args):
     torch.cuda.set_device(local)
     if world > 1:
         if args.backend == "nccl":
-            # the communicator log (rank count, transports, NVLS) goes to a file: stdout carries the one JSON line
+            # the communicator log (rank count, transports, NVLS) goes to stderr, where the driver reads it; stdout
+            # carries the one JSON line
             os.environ.setdefault("NCCL_DEBUG", "INFO")
             os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
-            os.environ.setdefault("NCCL_DEBUG_FILE", os.path.join(tempfile.gettempdir(), "grim_bench_nccl_%h_%p.log"))
             dist.init_process_group("nccl", device_id=torch.device("cuda", local))
         else:
             dist.init_process_group("gloo")
@@ -270,9 +274,6 @@ def run_ours(args):
     dt = slab.choose_dt(dP)                      # CFL 0.5 on the initial data, min over ranks; then held fixed
     zones = g.zones
     pbytes = dP.numel() * 8
-    # the pipelined host path (1 GPU, 3-D) moves the interior X^3 planes only; the ghost planes are filled on the device
-    pipelined = world == 1 and args.dim == 3 and g.n[2] >= 64 and zones >= 1500000 and not args.flux_ct
-    e2e_bytes = pbytes * g.n[2] // g.sz[2] if pipelined else pbytes
 
     def barrier():
         if world > 1:
@@ -285,14 +286,15 @@ def run_ours(args):
     l0 = g.launch_count()
     g.set_timing(True)
     sampler = ClockSampler(local) if rank == 0 else None
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     barrier()
-    e0.record()
-    for _ in range(args.steps):
+    ev[0].record()
+    for k in range(args.steps):
         slab.timestep(dP, dt)
-    e1.record()
+        ev[k + 1].record()                       # one event between steps: value stays the mean over the whole region
     barrier()
-    ms = e0.elapsed_time(e1)
+    ms = ev[0].elapsed_time(ev[args.steps])
+    per_step = sorted(ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps))
     clocks = sampler.stop() if sampler else None
     timing = g.get_timing()
     g.set_timing(False)
@@ -311,11 +313,16 @@ def run_ours(args):
             slab.timestep_host(hP, dt)
         barrier()
         e2e_s = (time.perf_counter() - t0) / e2e_steps
+    # the pipelined host path moves the interior X^3 planes only (the ghost planes are filled on the device); which form
+    # the call took is the library's decision (grid, arguments, GRIM_HOST_PIPELINE), so ask it
+    pipelined = world == 1 and g.last_host_mode() == "pipelined"
+    e2e_bytes = pbytes * g.n[2] // g.sz[2] if pipelined else pbytes
 
-    tmax = torch.tensor([ms, e2e_s], dtype=torch.float64, device="cuda")
+    med = per_step[len(per_step) // 2] if per_step else float("nan")
+    tmax = torch.tensor([ms, e2e_s, med, per_step[0] if per_step else float("nan")], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms, e2e_s = float(tmax[0]), float(tmax[1])
+    ms, e2e_s, ms_median, ms_min = (float(x) for x in tmax)
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -340,7 +347,8 @@ def run_ours(args):
     flux_hbm = ALG_BYTES_PER_ZONE_STAGE_FLUX * zones / (flux_ms * 1e-3) / 1e9
     line = {
         "metric": METRIC, "value": zones * world * args.steps / (ms * 1e-3), "unit": UNIT, "n_gpus": world,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps, "higher_is_better": True,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+        "ms_per_step_median": ms_median, "ms_per_step_min": ms_min, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": "config3-emhd-mp5-llf-minkowski-%d^%d%s" % (n, args.dim, ("-fluxct" if args.flux_ct else "") + ("-reduced7" if args.reduced else "")),
                    "zones_per_gpu": zones,
@@ -348,7 +356,7 @@ def run_ours(args):
                              "constants, fused Newton solve)", "dt": "fixed: CFL 0.5 on the initial data",
                    "l2": "inputs (%.2f GB per field) larger than L2" % (pbytes / 1e9),
                    "parallelism": "slab%d" % world, "backend": args.backend if world > 1 else None,
-                   "nccl_log": os.environ.get("NCCL_DEBUG_FILE") if (world > 1 and args.backend == "nccl") else None},
+                   "nccl_log": "stderr (NCCL_DEBUG=INFO, INIT)" if (world > 1 and args.backend == "nccl") else None},
         "clocks": clocks,
         "e2e": {"value": zones * world / e2e_s, "unit": UNIT, "h2d_bytes_per_step": e2e_bytes,
                 "d2h_bytes_per_step": e2e_bytes,
@@ -364,6 +372,8 @@ def run_ours(args):
             "peak_measured": probe, "peak_measured_source": "grim_fp64_probe (DFMA, 8 chains/thread), this run",
             "frac_of_measured": alu_ach / probe,
             "alg_fp64_instr_per_zone_stage": ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON * it_scale,
+            "executed_fp64_instr_per_zone_stage": EXECUTED_FP64_INSTR_PER_ZONE_STAGE_NEWTON * it_scale,
+            "frac_executed": alu_ach / alu_peak * EXECUTED_FP64_INSTR_PER_ZONE_STAGE_NEWTON / ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON,
             "mean_newton_iterations": mean_it, "launch_ms": newton_ms, "launches": int(nk_n)},
         "roofline_hbm": None if not headline else {
             "bound": "hbm", "kernel": NEWTON_KERNEL, "achieved": hbm_ach,

@@ -37,7 +37,7 @@
 extern "C" {
 #endif
 
-#define GRIM_VERSION 100
+#define GRIM_VERSION 101   /* 101: grim_grid_desc gained `closure`; binding.py refuses a library of another version */
 
 /* error codes */
 enum { GRIM_OK = 0, GRIM_EINVAL = -1, GRIM_ECUDA = -2, GRIM_ENOMEM = -3, GRIM_ESTATE = -4 };
@@ -210,6 +210,10 @@ int grim_set_metric_tables(grim_ctx *c, const double *tab, const double *conn);
 int grim_get_geometry(grim_ctx *c, int32_t loc, int64_t idx2d, double *gcov, double *gcon, double *sqrtmg,
                       double *alpha, double *tau, double *conn);
 
+/* ---- diagnostic entry points (measurement and self-test hooks; not steps of the path) ------------------------
+ * grim_fp64_probe, grim_arith_selftest here, grim_launch_count / grim_set_timing / grim_get_timing at the end of
+ * this header. */
+
 /* fp64 pipe probe: runs `iters` dependent-chain-free DFMA (fma=1) or DMUL+DADD (fma=0) instructions per thread
  * on a full grid and returns fp64 instructions per second (host out).  Used for the ALU roofline denominator. */
 int grim_fp64_probe(grim_ctx *c, int32_t fma, int32_t iters, double *inst_per_s);
@@ -236,6 +240,11 @@ int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t wide, int6
  *                                 grid allows it, regardless of size.
  *   grim_invert_primitives_host : U_host, P_host N*nz; iters/status/resnorm host outputs (may be NULL). */
 int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, double dt, double *dt_used);
+/* Which of the two forms the context's last grim_timestep_host call took (it depends on the grid, on the arguments and
+ * on GRIM_HOST_PIPELINE, see above): callers that account for the bytes copied, or that rely on the ghost zones of
+ * P_host having been copied, read it here instead of re-deriving the rule.  Host bookkeeping, no device work. */
+enum { GRIM_HOST_MODE_NONE = 0, GRIM_HOST_MODE_WHOLE = 1, GRIM_HOST_MODE_PIPELINED = 2 };
+int grim_last_host_mode(const grim_ctx *c);
 int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, double *P_host, int32_t *iters_host,
                                 int32_t *status_host, double *resnorm_host);
 
@@ -278,10 +287,10 @@ int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, d
 int grim_invert_primitives_static(const grim_grid_desc *d, int64_t nz, const double *U_target, const double *geom,
                                   double *P_inout, int32_t *iters, int32_t *status, double *resnorm);
 
-/* Number of kernels the library has launched on this context since creation (host bookkeeping). */
+/* Diagnostic: number of kernels the library has launched on this context since creation (host bookkeeping). */
 int64_t grim_launch_count(const grim_ctx *c);
 
-/* Per-kernel-class device timing for the roofline report (bench.py): while on, every launch group is bracketed by
+/* Diagnostic: per-kernel-class device timing for the roofline report (bench.py): while on, every launch group is bracketed by
  * a CUDA event pair on the context's stream.  grim_set_timing(on != 0) clears the accumulators; grim_get_timing
  * waits for the recorded events and returns, per class, the summed device milliseconds and the launch count
  * (host out, GRIM_NKCLASS entries each, may be NULL).  Classes: */

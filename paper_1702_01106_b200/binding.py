@@ -62,6 +62,7 @@ _SIGNATURES = {
     "grim_fp64_probe": (C.c_int, [_vp, _i32, _i32, _pd]),
     "grim_arith_selftest": (C.c_int, [_vp, _i64, _i64, _i32, _pi64]),
     "grim_timestep_host": (C.c_int, [_vp, _vp, _i32, _dbl, _pd]),
+    "grim_last_host_mode": (C.c_int, [_vp]),
     "grim_invert_primitives_host": (C.c_int, [_vp, _i64, _vp, _vp, _vp, _vp, _vp]),
     "grim_invert_primitives_static": (C.c_int, [C.POINTER(GridDesc), _i64, _vp, _vp, _vp, _vp, _vp, _vp]),
     "grim_launch_count": (_i64, [_vp]),
@@ -70,6 +71,8 @@ _SIGNATURES = {
 }
 
 KERNEL_CLASSES = ("ghosts", "flux", "newton", "invert", "other")
+HOST_MODES = ("none", "whole", "pipelined")      # GRIM_HOST_MODE_*
+ABI_VERSION = 101                                # GRIM_VERSION this file's ctypes layouts (GridDesc, StepStats) mirror
 
 
 def exported_symbols():
@@ -92,6 +95,10 @@ def lib():
             raise GrimError("%s is missing: build it with `python -m paper_1702_01106_b200.build` "
                             "(there is no CPU fallback)" % p)
         L = C.CDLL(p)
+        L.grim_version.restype = C.c_int
+        if L.grim_version() != ABI_VERSION:
+            raise GrimError("%s is version %d, this binding mirrors the structs of version %d: rebuild it with "
+                            "`python -m paper_1702_01106_b200.build --force`" % (p, L.grim_version(), ABI_VERSION))
         for name, (res, args) in _SIGNATURES.items():
             f = getattr(L, name)
             f.restype = res
@@ -324,6 +331,10 @@ class Grid:
         self._check(self._L.grim_timestep_host(self.h, _host_ptr(P_host, self.torch.float64), nsteps, dt,
                                                C.byref(dtu)), "grim_timestep_host")
         return dtu.value
+
+    def last_host_mode(self):
+        """'none' | 'whole' | 'pipelined': the form the last timestep_host call took (grim_last_host_mode)."""
+        return HOST_MODES[self._L.grim_last_host_mode(self.h)]
 
     def get_geometry(self, loc, j, i):
         import numpy as np

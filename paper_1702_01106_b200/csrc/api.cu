@@ -45,7 +45,7 @@ struct grim_ctx {
   StatsDev *stats;             // device, 2 stages
   double *probe_sink;
   long long *list[2];          // inversion active lists
-  long long list_cap;
+  long long list_cap[2];   // capacity, in zones, of list[0] (stage sweeps and inversion) and list[1] (inversion only)
   double *hostP;               // staging for the *_host entry points
   cudaStream_t s_in, s_out;    // copy streams of the pipelined grim_timestep_host
   cudaStream_t s_st2;          // its second compute stream (stage 2 of a slab beside stage 1 of a later one)
@@ -53,6 +53,7 @@ struct grim_ctx {
   double *invbuf;              // U, P, resnorm, iters, status of grim_invert_primitives_host
   long long invbuf_nz;
   int64_t launches;
+  int last_host_mode;          // what the last grim_timestep_host call did: GRIM_HOST_MODE_*
   int no_pipeline;             // GRIM_HOST_PIPELINE in the environment: 1 = "0" (never), -1 = "1" (always), 0 = unset
   // sweep policy of solve_stage: the deferred-zone counts of the recent sweep-mode solves arrive asynchronously in
   // pinned host memory; a run whose solves never defer a zone (smooth data) goes back to single launches and probes again
@@ -411,6 +412,17 @@ extern "C" int grim_newton_step(grim_ctx *c, const double *P_n, const double *P_
   return GRIM_OK;
 }
 
+// Grows active-zone list a to hold n zone indices (never shrinks).
+static int ensure_list(grim_ctx *c, int a, long long n) {
+  if (c->list_cap[a] >= n) return GRIM_OK;
+  if (c->list[a]) cudaFree(c->list[a]);
+  c->list[a] = nullptr;
+  c->list_cap[a] = 0;
+  CU(cudaMalloc((void **)&c->list[a], (size_t)n * sizeof(long long)));
+  c->list_cap[a] = n;
+  return GRIM_OK;
+}
+
 // A fresh solve of every interior zone to a terminal status (steps a4-a7), in sweeps: the first launch gives every zone
 // GRIM_STAGE_SWEEP iterations; the zones that need more -- a few per cent in a run whose iteration counts spread (the
 // torus: 2-8), none in a smooth run -- are collected and solved afresh, to the end, by a second launch over that list
@@ -443,10 +455,13 @@ static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const 
       }
     }
     for (int q = 0; q < 4; q++) {
-      if (c->sweep_pending[q] && cudaEventQuery(c->sweep_ev[q]) == cudaSuccess) {
+      if (!c->sweep_pending[q]) continue;
+      if (cudaEventQuery(c->sweep_ev[q]) == cudaSuccess) {
         c->sweep_pending[q] = 0;
         if (c->sweep_counts[q] == 0) c->sweep_quiet++;
         else c->sweep_quiet = 0;
+      } else {
+        (void)cudaGetLastError();  // cudaErrorNotReady is an answer, not a failure: keep it out of check_launch()
       }
     }
     if (c->sweep_quiet >= 4) {
@@ -458,13 +473,9 @@ static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const 
       sweeps = false;
     }
   }
-  if (sweeps && c->list_cap < gv.nint) {
-    for (int a = 0; a < 2; a++) {
-      if (c->list[a]) cudaFree(c->list[a]);
-      c->list[a] = nullptr;
-      CU(cudaMalloc((void **)&c->list[a], (size_t)gv.nint * sizeof(long long)));
-    }
-    c->list_cap = gv.nint;
+  if (sweeps) {
+    int rcl = ensure_list(c, 0, gv.nint);  // the stage solve compacts once: one list
+    if (rcl) return rcl;
   }
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
   GridView g1 = gv;
@@ -519,13 +530,9 @@ extern "C" int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_t
     return fail(c, GRIM_EINVAL, "grim_invert_primitives: bad argument");
   if (nz == 0) return GRIM_OK;
   CU(cudaSetDevice(c->d.device));
-  if (c->list_cap < nz) {
-    for (int a = 0; a < 2; a++) {
-      if (c->list[a]) cudaFree(c->list[a]);
-      c->list[a] = nullptr;
-      CU(cudaMalloc((void **)&c->list[a], (size_t)nz * sizeof(long long)));
-    }
-    c->list_cap = nz;
+  for (int a = 0; a < 2; a++) {  // the inversion ping-pongs between two lists
+    int rcl = ensure_list(c, a, nz);
+    if (rcl) return rcl;
   }
   // sweeps of a few iterations each over the compacted set of zones that are still iterating
   const int kmax = c->gv.sp.kmax;
@@ -703,16 +710,16 @@ extern "C" int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t
 // kernels of slab c (stage 1) and c - 1 (stage 2) and the device -> host copy of slab c - 2 run at the same time on three
 // streams.  A slab's stage 1 needs P_n of the neighbouring slabs (stencil of the flux step, 3 + 1 planes), its stage 2
 // P_{n+1/2} of the neighbouring slabs; the X^3 boundary (periodic wrap or a physical boundary) couples the first and
-// the last slab, which therefore arrive first and finish last.  All kernels run on the context's stream in an order
-// that keeps every read ahead of the write that would overwrite it (stage 2 writes P_{n+1} over P_n in place); the
-// results are those of grim_timestep bit for bit.  Ghost zones of P_host are neither read nor written.
+// the last slab, which therefore arrive first and finish last.  Stage 1 of every slab runs on the context's stream, stage 2
+// on a second compute stream (s_st2), ordered by events so that every read stays ahead of the write that would overwrite
+// it (stage 2 writes P_{n+1} over P_n in place); the results are those of grim_timestep bit for bit.  Ghost zones of P_host are neither read nor written.
 #ifndef GRIM_HOST_SLABS
 #define GRIM_HOST_SLABS 16
 #endif
 #ifndef GRIM_HOST_EDGE
 #define GRIM_HOST_EDGE 4
 #endif
-static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
+static int pipelined_enqueue(grim_ctx *c, double *P_host, double dt) {
   const GridView &gv = c->gv;
   cudaStream_t s = c->stream;
   const int K = GRIM_HOST_SLABS, ng = gv.ngd[2], n3 = gv.n[2];
@@ -753,11 +760,16 @@ static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
   CU(cudaStreamWaitEvent(c->s_in, c->ev_in[K], 0));
   CU(cudaStreamWaitEvent(c->s_out, c->ev_in[K], 0));
   CU(cudaStreamWaitEvent(s2, c->ev_in[K], 0));
+  // the lambdas cannot return through CU(): they keep the first failing return code, checked at the end
+  cudaError_t bad = cudaSuccess;
+  auto keep = [&](cudaError_t e) {
+    if (e != cudaSuccess && bad == cudaSuccess) bad = e;
+  };
   auto h2d = [&](int q) {
     const size_t off = (size_t)(ng + k0[q]) * plane;
-    cudaMemcpy2DAsync(d + off, pitch, P_host + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
-                      cudaMemcpyHostToDevice, c->s_in);
-    cudaEventRecord(c->ev_in[q], c->s_in);
+    keep(cudaMemcpy2DAsync(d + off, pitch, P_host + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
+                           cudaMemcpyHostToDevice, c->s_in));
+    keep(cudaEventRecord(c->ev_in[q], c->s_in));
   };
   h2d(K - 1);
   for (int q = 0; q < K - 1; q++) h2d(q);
@@ -786,14 +798,14 @@ static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
   // slab-wise launches overlap instead of adding up.
   auto stage2 = [&](int q, cudaEvent_t after) {
     const GridView g = slab(q);
-    cudaStreamWaitEvent(s2, after, 0);
+    keep(cudaStreamWaitEvent(s2, after, 0));
     c->launches += timed(c, GRIM_K_FLUX, [&] { return launch_fluxes(g, c->Ph, d, dt, c->C, c->G, c->Fface, c->cface, nullptr, s2); }, s2);
     c->launches += timed(c, GRIM_K_NEWTON, [&] { return launch_newton_stage(g, d, c->Ph, c->C, c->G, c->Ph, 1, dt, 0, d, c->resnorm, c->status, c->iters, c->cnt, s2); }, s2);
-    cudaEventRecord(c->ev_done[q], s2);
-    cudaStreamWaitEvent(c->s_out, c->ev_done[q], 0);
+    keep(cudaEventRecord(c->ev_done[q], s2));
+    keep(cudaStreamWaitEvent(c->s_out, c->ev_done[q], 0));
     const size_t off = (size_t)(ng + k0[q]) * plane;
-    cudaMemcpy2DAsync(P_host + off, pitch, d + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
-                      cudaMemcpyDeviceToHost, c->s_out);
+    keep(cudaMemcpy2DAsync(P_host + off, pitch, d + off, pitch, (size_t)(k0[q + 1] - k0[q]) * plane * 8, (size_t)gv.nvar,
+                           cudaMemcpyDeviceToHost, c->s_out));
   };
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
   CU(cudaStreamWaitEvent(s, c->ev_in[K - 1], 0));
@@ -815,10 +827,20 @@ static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
   CU(cudaEventRecord(c->ev_s1[K], s));
   stage2(K - 1, c->ev_s1[K]);
   stage2(0, c->ev_s1[K]);
-  int rc = check_launch(c, "pipelined timestep");
-  CU(cudaStreamSynchronize(c->s_out));
-  CU(cudaStreamSynchronize(s2));
-  CU(cudaStreamSynchronize(s));
+  if (bad != cudaSuccess) return fail(c, GRIM_ECUDA, std::string("pipelined timestep: ") + cudaGetErrorString(bad));
+  return check_launch(c, "pipelined timestep");
+}
+
+// Enqueues the pipelined step and waits for it.  Whatever pipelined_enqueue returns -- also an early error return with
+// copies into the caller's P_host still in flight -- all four streams are drained before the caller gets control back.
+static int timestep_host_pipelined(grim_ctx *c, double *P_host, double dt) {
+  int rc = pipelined_enqueue(c, P_host, dt);
+  cudaStream_t side[3] = {c->s_in, c->s_st2, c->s_out};
+  for (int q = 0; q < 4; q++) {
+    if (q < 3 && side[q] == nullptr) continue;  // a side stream that was never created
+    cudaError_t e = cudaStreamSynchronize(q < 3 ? side[q] : c->stream);
+    if (e != cudaSuccess && rc == GRIM_OK) rc = fail(c, GRIM_ECUDA, std::string("pipelined timestep: ") + cudaGetErrorString(e));
+  }
   return rc;
 }
 
@@ -838,11 +860,13 @@ extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, d
     const bool big = c->gv.nint >= 1500000 || c->no_pipeline < 0;
     if (nsteps == 1 && dt > 0.0 && c->gv.dim == 3 && c->gv.n[2] >= 4 * GRIM_HOST_SLABS && !c->gv.flux_ct && !caller_ghosts &&
         big && c->no_pipeline <= 0) {
+      c->last_host_mode = GRIM_HOST_MODE_PIPELINED;
       rc = timestep_host_pipelined(c, P_host, dt);
       if (rc == GRIM_OK && dt_used) *dt_used = dt;
       return rc;
     }
   }
+  c->last_host_mode = GRIM_HOST_MODE_WHOLE;
   CU(cudaMemcpyAsync(c->hostP, P_host, pbytes, cudaMemcpyHostToDevice, c->stream));
   for (int s = 0; s < nsteps; s++) {
     rc = grim_timestep(c, c->hostP, dt, dt_used, nullptr);
@@ -852,6 +876,8 @@ extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, d
   CU(cudaStreamSynchronize(c->stream));
   return GRIM_OK;
 }
+
+extern "C" int grim_last_host_mode(const grim_ctx *c) { return c ? c->last_host_mode : GRIM_HOST_MODE_NONE; }
 
 extern "C" int grim_invert_primitives_host(grim_ctx *c, int64_t nz, const double *U_host, double *P_host,
                                            int32_t *iters_host, int32_t *status_host, double *resnorm_host) {

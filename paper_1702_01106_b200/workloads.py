@@ -220,7 +220,8 @@ def fm_torus(n1=256, n2=256, n3=1, nvar=10, a=0.9375, h=0.3, r_in=6.0, r_max=12.
              beta=100.0, seed_field=1e-5, noise=0.04, noise_phi=0.02, seed=9375, rho_floor=1e-4, u_floor=1e-6):
     """BASELINE config 4 (n3 = 1) / config 5 (n3 > 1): the equilibrium torus of the derivation above with inner edge
     r_in and pressure maximum r_max on an MKS grid (h = 0.3), X1 = ln r in [ln 1.3, ln 40], X2 in [0, 1], outflow /
-    polar reflection / periodic boundaries, tau_R = r^{3/2}, closure coefficients 1, MP5; polytrope p = kappa rho^gam
+    polar reflection / periodic boundaries, tau_R = r^{3/2}, closure coefficients 1, generalised minmod (theta = 1; reading
+    C-25: an MP5 torus run waits for floors and limiters the paper does not print, see below); polytrope p = kappa rho^gam
     normalised to rho = 1 at the pressure maximum; outside it a static atmosphere rho_floor r^{-3/2}, u_floor r^{-5/2};
     single poloidal field loop A_phi = max(rho - 0.2, 0) scaled to 2 max(P_g) / max(b^2) = beta, plus a weak uniform
     vertical seed field (A_phi += seed_field r^2 sin^2 theta / 2) so that bhat (eqs 33-34) is defined everywhere;

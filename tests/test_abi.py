@@ -32,7 +32,7 @@ def test_exports_every_declared_symbol(L):
 
 
 def test_version_and_struct_layout(L):
-    assert L.grim_version() == 100
+    assert L.grim_version() == 101
     # the structs the binding marshals must have the layout a C compiler gives include/grim.h
     import subprocess
     import tempfile

@@ -22,6 +22,7 @@ def _check(gk, P0, steps=2):
     gc.fill_ghosts(dP)
     dt, _ = gc.timestep(dP.clone(), 0.0, want_dt=True)
     hP = torch.from_numpy(P0.copy()).pin_memory()
+    assert gc.last_host_mode() == "none"
     l0 = gc.launch_count()
     for _ in range(steps):
         gc.timestep(dP, dt)
@@ -30,6 +31,7 @@ def _check(gk, P0, steps=2):
     for _ in range(steps):
         gc.timestep_host(hP, 1, dt)
     assert (gc.launch_count() - l0) // steps > 4 * per_step          # the slab-wise launches did run
+    assert gc.last_host_mode() == "pipelined"
     assert torch.equal(gc.interior(hP), gc.interior(dP).cpu())
     # pageable host memory takes the same path
     hQ = torch.from_numpy(P0.copy())
@@ -39,6 +41,7 @@ def _check(gk, P0, steps=2):
     # several steps per call: copy in, step, copy out (not pipelined), same result
     hR = torch.from_numpy(P0.copy())
     gc.timestep_host(hR, steps, dt)
+    assert gc.last_host_mode() == "whole"
     assert torch.equal(gc.interior(hR), gc.interior(dP).cpu())
 
 
