@@ -30,8 +30,7 @@ UNIT = "zone-updates/s"
 # Algorithmic fp64 work: DADD + DMUL + DFMA thread instructions that the method's definition requires under the strict
 # arithmetic contract (every + - * separately rounded, / and sqrt as correctly rounded Newton-Raphson sequences), counted
 # with ncu on the round's first kernel (profiles/r1a_ncu_full_stage_kernels_baseline.md) and then FROZEN, so that later
-# kernels cannot raise the fraction by executing more instructions.  (The current kernel executes 6242 fp64-pipe thread
-# instructions per zone and stage, compares included: profiles/r1g_ncu_full_stage_kernels.md.)
+# kernels cannot raise the fraction by executing more instructions.  (What the current kernel executes: EXECUTED_FP64_INSTR_PER_ZONE_STAGE_NEWTON below.)
 ALG_FP64_INSTR_PER_ZONE_STAGE_NEWTON = 6114.0
 ALG_BYTES_PER_ZONE_STAGE_NEWTON = 8.0 * (10 + 10 + 10 + 10 + 3 + 10 + 1) + 4 * 4   # P^k,P_n,P_E,C,G in; P,|R| out; status,iters in/out
 # dram__bytes_read.sum + dram__bytes_write.sum of the Newton kernel per zone, mean of the stage-1 and stage-2 launches
@@ -47,7 +46,7 @@ NCU_TRAFFIC_SOURCE = "profiles/r2c_final_kernels.md"
 # 8(d) "Flux + stage constant, EMHD": P_E 10 (x 1.3-1.5 halo re-read) + P_n 10 in, C 10 + G 3 out -> 320-400 B; the
 # upper figure.  Algorithmic fp64 work: DADD + DMUL + DFMA thread instructions of the same four kernels in the round's
 # capture of the round-1 kernels (3997 per zone-stage: 3 x 1084 face + 744 stage constant; profiles/r2c_final_kernels.md
-# and r2b_optimisation_log.md), frozen like the Newton count.
+# and DESIGN.md 13.3), frozen like the Newton count.
 ALG_BYTES_PER_ZONE_STAGE_FLUX = 400.0
 ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX = 3997.0
 NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX = 1075.0

@@ -15,12 +15,7 @@
 using namespace grim;
 
 // grim_invert_primitives: Newton iterations per sweep over the compacted active set (first sweep, later sweeps)
-#ifndef GRIM_SWEEP_FIRST
-#define GRIM_SWEEP_FIRST 4
-#endif
-#ifndef GRIM_SWEEP_REST
-#define GRIM_SWEEP_REST 4
-#endif
+static constexpr int SWEEP_FIRST = 4, SWEEP_REST = 4;
 
 struct KernelSpan {
   int kclass, launches;
@@ -57,7 +52,7 @@ struct grim_ctx {
   int no_pipeline;             // GRIM_HOST_PIPELINE in the environment: 1 = "0" (never), -1 = "1" (always), 0 = unset
   // sweep policy of solve_stage: the deferred-zone counts of the recent sweep-mode solves arrive asynchronously in
   // pinned host memory; a run whose solves never defer a zone (smooth data) goes back to single launches and probes again
-  // every GRIM_SWEEP_PROBE solves
+  // every SWEEP_PROBE solves
   unsigned long long *sweep_counts;  // pinned, SWEEP_RING entries
   cudaEvent_t sweep_ev[4];
   int sweep_pending[4];
@@ -424,21 +419,17 @@ static int ensure_list(grim_ctx *c, int a, long long n) {
 }
 
 // A fresh solve of every interior zone to a terminal status (steps a4-a7), in sweeps: the first launch gives every zone
-// GRIM_STAGE_SWEEP iterations; the zones that need more -- a few per cent in a run whose iteration counts spread (the
+// STAGE_SWEEP iterations; the zones that need more -- a few per cent in a run whose iteration counts spread (the
 // torus: 2-8), none in a smooth run -- are collected and solved afresh, to the end, by a second launch over that list
 // only, so that a warp does not idle through the long solves of a few of its lanes.  The per-zone results are those of
 // one uninterrupted solve (it IS one, for every zone); the list length stays on the device.
-#ifndef GRIM_STAGE_SWEEP
-#define GRIM_STAGE_SWEEP 4
-#endif
-#ifndef GRIM_SWEEP_PROBE
-#define GRIM_SWEEP_PROBE 64
-#endif
+static constexpr int STAGE_SWEEP = 4;   // iterations of the first launch (3 and 5 measured slower on the torus)
+static constexpr int SWEEP_PROBE = 64;  // single-launch solves between two probes of the sweep mode
 static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const double *PE, const double *C,
                        const double *G, const double *Pguess, double dt_stage, double *Pout, double *resnorm,
                        int32_t *status, int32_t *iters) {
   cudaStream_t s = c->stream;
-  bool sweeps = GRIM_STAGE_SWEEP > 0 && gv.sp.kmax > GRIM_STAGE_SWEEP;
+  bool sweeps = STAGE_SWEEP > 0 && gv.sp.kmax > STAGE_SWEEP;
   // While the stream is being captured into a CUDA graph the policy below (event queries, a pinned read-back) must not
   // run: a captured step always takes the two-launch form, whose list length stays on the device.
   cudaStreamCaptureStatus cap = cudaStreamCaptureStatusNone;
@@ -466,7 +457,7 @@ static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const 
     }
     if (c->sweep_quiet >= 4) {
       c->sweep_quiet = 0;
-      c->sweep_skip = GRIM_SWEEP_PROBE;
+      c->sweep_skip = SWEEP_PROBE;
     }
     if (c->sweep_skip > 0) {
       c->sweep_skip--;
@@ -479,7 +470,7 @@ static int solve_stage(grim_ctx *c, const GridView &gv, const double *Pn, const 
   }
   CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), s));
   GridView g1 = gv;
-  if (sweeps) g1.sp.kmax = GRIM_STAGE_SWEEP;
+  if (sweeps) g1.sp.kmax = STAGE_SWEEP;
   c->launches += timed(c, GRIM_K_NEWTON, [&] {
     return launch_newton_stage(g1, Pn, PE, C, G, Pguess, 1, dt_stage, 0, Pout, resnorm, status, iters, c->cnt, s, nullptr, 0,
                                sweeps ? c->list[0] : nullptr);
@@ -539,7 +530,7 @@ extern "C" int grim_invert_primitives(grim_ctx *c, int64_t nz, const double *U_t
   long long nlist = nz;
   int first = 1, cur = 0, done_iters = 0;
   while (nlist > 0) {
-    const int sweep = first ? GRIM_SWEEP_FIRST : GRIM_SWEEP_REST;
+    const int sweep = first ? SWEEP_FIRST : SWEEP_REST;
     CU(cudaMemsetAsync(c->cnt, 0, sizeof(Counters), c->stream));
     c->launches += timed(c, GRIM_K_INVERT, [&] { return launch_invert(c->gv, nz, nlist, c->list[cur], U_target, geom, P_inout, iters, status, resnorm, sweep,
                                  first, c->list[cur ^ 1], c->cnt, c->stream); });
@@ -713,16 +704,12 @@ extern "C" int grim_arith_selftest(grim_ctx *c, int64_t n, int64_t seed, int32_t
 // the last slab, which therefore arrive first and finish last.  Stage 1 of every slab runs on the context's stream, stage 2
 // on a second compute stream (s_st2), ordered by events so that every read stays ahead of the write that would overwrite
 // it (stage 2 writes P_{n+1} over P_n in place); the results are those of grim_timestep bit for bit.  Ghost zones of P_host are neither read nor written.
-#ifndef GRIM_HOST_SLABS
-#define GRIM_HOST_SLABS 16
-#endif
-#ifndef GRIM_HOST_EDGE
-#define GRIM_HOST_EDGE 4
-#endif
+static constexpr int HOST_SLABS = 16;  // slabs of the pipelined host step
+static constexpr int HOST_EDGE = 4;    // planes of its first and last slab
 static int pipelined_enqueue(grim_ctx *c, double *P_host, double dt) {
   const GridView &gv = c->gv;
   cudaStream_t s = c->stream;
-  const int K = GRIM_HOST_SLABS, ng = gv.ngd[2], n3 = gv.n[2];
+  const int K = HOST_SLABS, ng = gv.ngd[2], n3 = gv.n[2];
   const size_t plane = (size_t)gv.sz[0] * gv.sz[1], pitch = (size_t)gv.zg * 8;
   if (!c->s_in) CU(cudaStreamCreateWithFlags(&c->s_in, cudaStreamNonBlocking));
   if (!c->s_out) CU(cudaStreamCreateWithFlags(&c->s_out, cudaStreamNonBlocking));
@@ -737,12 +724,12 @@ static int pipelined_enqueue(grim_ctx *c, double *P_host, double dt) {
     c->ev_s1.push_back(e);
   }
   cudaStream_t s2 = c->s_st2;
-  int k0[GRIM_HOST_SLABS + 1];
+  int k0[HOST_SLABS + 1];
   // Slab boundaries, multiples of the 4-plane flux tiles.  The first and the last slab are coupled through the X^3
-  // boundary: they arrive first and finish last, nothing overlaps their copies -- so they are thin (GRIM_HOST_EDGE
+  // boundary: they arrive first and finish last, nothing overlaps their copies -- so they are thin (HOST_EDGE
   // planes) and the K - 2 slabs between them share the rest.
   {
-    const int e = (n3 >= 16 * GRIM_HOST_EDGE) ? GRIM_HOST_EDGE : 0;
+    const int e = (n3 >= 16 * HOST_EDGE) ? HOST_EDGE : 0;
     if (e) {
       k0[0] = 0;
       k0[1] = e;
@@ -858,7 +845,7 @@ extern "C" int grim_timestep_host(grim_ctx *c, double *P_host, int32_t nsteps, d
         if (c->gv.ngd[a] > 0 && c->d.bc[a][sd] == GRIM_BC_NONE) caller_ghosts = true;
     // slab-wise launches pay off from about 1.5 M zones (measured: 64^3 and 96^3 are faster copied whole)
     const bool big = c->gv.nint >= 1500000 || c->no_pipeline < 0;
-    if (nsteps == 1 && dt > 0.0 && c->gv.dim == 3 && c->gv.n[2] >= 4 * GRIM_HOST_SLABS && !c->gv.flux_ct && !caller_ghosts &&
+    if (nsteps == 1 && dt > 0.0 && c->gv.dim == 3 && c->gv.n[2] >= 4 * HOST_SLABS && !c->gv.flux_ct && !caller_ghosts &&
         big && c->no_pipeline <= 0) {
       c->last_host_mode = GRIM_HOST_MODE_PIPELINED;
       rc = timestep_host_pipelined(c, P_host, dt);

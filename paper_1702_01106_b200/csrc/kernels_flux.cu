@@ -111,14 +111,10 @@ struct FaceTile {
   static constexpr int T0 = (DIR == 0) ? 128 : 32, T1 = (DIR == 1) ? 4 : 1, T2 = (DIR == 2) ? 4 : 1;
 };
 
-#ifndef GRIM_FLUX_MINB
-#define GRIM_FLUX_MINB 4
-#endif
-#ifndef GRIM_FLUX_MINB_GEN
-#define GRIM_FLUX_MINB_GEN 4
-#endif
+// resident blocks per SM the face kernels are compiled for (flat and general metric: 4 x 128 threads, 128 registers)
+static constexpr int FLUX_MINB = 4, FLUX_MINB_GEN = 4;
 template <int N, int RECON, class G, int DIR>  // DIR = 0..2
-__global__ void __launch_bounds__(FB, G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN)
+__global__ void __launch_bounds__(FB, G::flat ? FLUX_MINB : FLUX_MINB_GEN)
 face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE, double *__restrict__ Fface,
                  double *__restrict__ cface) {
   using T = FaceTile<DIR>;
@@ -169,20 +165,12 @@ face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__
   }
 }
 
-// The same tiles with the stencil zones brought in by TMA, one tile ahead of the arithmetic.  A block is persistent: it
-// takes the tiles b, b + gridDim.x, ...; while it computes the faces of one tile from buffer q, the bulk tensor copy of
-// the next tile's box -- all N variables, (T0 + halo) x (T1 + halo) x (T2 + halo) zones, out-of-range zones read as
-// zero -- lands in buffer 1 - q and signals that buffer's mbarrier.  One thread issues the copy; nobody computes
-// addresses or holds staging registers.  (A TMA box row starts on a 16-byte boundary and is a multiple of 16 bytes long:
-// the box starts at the even X^1 index at or below the first stencil zone and has an even X^1 extent.)
-#ifndef GRIM_FLUX_TMA
-#define GRIM_FLUX_TMA 1
-#endif
-// blocks per resident block slot: 1 = fully persistent; 0 = one tile per block (no prefetch, the copy only replaces the
-// per-thread staging loads)
-#ifndef GRIM_FLUX_TMA_WAVES
-#define GRIM_FLUX_TMA_WAVES 0
-#endif
+// The same tiles with the stencil zones brought in by TMA: one bulk tensor copy per block brings the tile's box -- all N
+// variables, (T0 + halo) x (T1 + halo) x (T2 + halo) zones, out-of-range zones read as zero -- into shared memory and
+// signals the block's mbarrier.  One thread issues the copy; nobody computes addresses or holds staging registers.  (A TMA
+// box row starts on a 16-byte boundary and is a multiple of 16 bytes long: the box starts at the even X^1 index at or
+// below the first stencil zone and has an even X^1 extent.)  One tile per block: with 4 resident blocks per SM the copies
+// of some blocks overlap the arithmetic of others; a persistent, double-buffered form measured slower.
 template <int RECON, int DIR>
 struct TmaTile {
   using T = FaceTile<DIR>;
@@ -198,66 +186,45 @@ __host__ __device__ constexpr size_t tma_tile_bytes() {
 }
 
 template <int N, int RECON, class G, int DIR>
-__global__ void __launch_bounds__(FB, G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN)
+__global__ void __launch_bounds__(FB, G::flat ? FLUX_MINB : FLUX_MINB_GEN)
 face_flux_tma_kernel(const __grid_constant__ GridView gv, const __grid_constant__ CUtensorMap tmap,
                      const double *__restrict__ PE, double *__restrict__ Fface, double *__restrict__ cface, int ntx,
-                     int nty, int ntz) {
+                     int nty) {
   using T = FaceTile<DIR>;
   using X = TmaTile<RECON, DIR>;
   constexpr uint32_t BYTES = (uint32_t)(N * X::EZ * sizeof(double));
   extern __shared__ __align__(128) unsigned char tma_smem[];
-  __shared__ uint64_t bar[2];
-  double *buf[2] = {(double *)tma_smem,
-                    (double *)(tma_smem + (GRIM_FLUX_TMA_WAVES == 0 ? 0 : tma_tile_bytes<N, RECON, DIR>()))};
-  const long long ntiles = (long long)ntx * nty * ntz;
+  __shared__ uint64_t bar;
+  double *buf = (double *)tma_smem;
+  const unsigned tl = blockIdx.x, nx = (unsigned)ntx, ny = (unsigned)nty;  // (the tile count fits 32 bits)
+  const int tx = (int)(tl % nx), ty = (int)((tl / nx) % ny), tz = (int)(tl / (nx * ny));
+  const int fi = gv.ngd[0] + tx * T::T0, fj = gv.ngd[1] + ty * T::T1, fk = gv.ngd[2] + gv.koff + tz * T::T2;
   if (threadIdx.x == 0) {
-    mbar_init(&bar[0], 1);
-    mbar_init(&bar[1], 1);
+    mbar_init(&bar, 1);
     mbar_init_fence();
+    mbar_expect_tx(&bar, BYTES);
+    tma_load_4d(buf, &tmap, &bar, (fi - (DIR == 0 ? X::LO : 0)) & ~1, fj - (DIR == 1 ? X::LO : 0),
+                fk - (DIR == 2 ? X::LO : 0), 0);
   }
   __syncthreads();
-  auto origin = [&](long long tile, int &fi, int &fj, int &fk) {
-    const unsigned tl = (unsigned)tile, nx = (unsigned)ntx, ny = (unsigned)nty;  // (the tile count fits 32 bits)
-    const int tx = (int)(tl % nx), ty = (int)((tl / nx) % ny), tz = (int)(tl / (nx * ny));
-    fi = gv.ngd[0] + tx * T::T0;
-    fj = gv.ngd[1] + ty * T::T1;
-    fk = gv.ngd[2] + gv.koff + tz * T::T2;
-  };
-  auto issue = [&](long long tile, int q) {  // one thread
-    int fi, fj, fk;
-    origin(tile, fi, fj, fk);
-    mbar_expect_tx(&bar[q], BYTES);
-    tma_load_4d(buf[q], &tmap, &bar[q], (fi - (DIR == 0 ? X::LO : 0)) & ~1, fj - (DIR == 1 ? X::LO : 0),
-                fk - (DIR == 2 ? X::LO : 0), 0);
-  };
   const int xshift = (gv.ngd[0] - (DIR == 0 ? X::LO : 0)) & 1;  // tile origins advance by an even T0
   const int t0 = (int)threadIdx.x % T::T0, t1 = ((int)threadIdx.x / T::T0) % T::T1,
             t2 = (int)threadIdx.x / (T::T0 * T::T1);
-  if (threadIdx.x == 0 && (long long)blockIdx.x < ntiles) issue(blockIdx.x, 0);
-  int it = 0;
-  for (long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x, it++) {
-    const int q = it & 1;
-    // buffer 1 - q was released by the block-wide sync that ended the previous iteration
-    if (threadIdx.x == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x, q ^ 1);
-    mbar_wait(&bar[q], (uint32_t)((it >> 1) & 1));
-    int fi, fj, fk;
-    origin(tile, fi, fj, fk);
-    const int i = fi + t0, j = fj + t1, k = fk + t2;
-    if (i < gv.ngd[0] + gv.n[0] && j < gv.ngd[1] + gv.n[1] && k < gv.ngd[2] + gv.koff + gv.n[2]) {
-      const long long z = zone_index(gv, i, j, k);
-      SpecArith ar;
-      double F[N], c;
-      const TileStencil<X::EZ, X::MS> st{buf[q] + (t2 * X::E1 + t1) * X::E0 + t0 + xshift};
-      face_compute<N, RECON, G, DIR>(ar, gv, st, i, j, F, c);
-      if (ar.good()) {
+  mbar_wait(&bar, 0);
+  const int i = fi + t0, j = fj + t1, k = fk + t2;
+  if (i < gv.ngd[0] + gv.n[0] && j < gv.ngd[1] + gv.n[1] && k < gv.ngd[2] + gv.koff + gv.n[2]) {
+    const long long z = zone_index(gv, i, j, k);
+    SpecArith ar;
+    double F[N], c;
+    const TileStencil<X::EZ, X::MS> st{buf + (t2 * X::E1 + t1) * X::E0 + t0 + xshift};
+    face_compute<N, RECON, G, DIR>(ar, gv, st, i, j, F, c);
+    if (ar.good()) {
 #pragma unroll
-        for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
-        cface[z] = c;
-      } else {
-        face_replay<N, RECON, G, DIR>(gv, PE, z, i, j, Fface, cface);
-      }
+      for (int v = 0; v < N; v++) Fface[v * gv.zg + z] = F[v];
+      cface[z] = c;
+    } else {
+      face_replay<N, RECON, G, DIR>(gv, PE, z, i, j, Fface, cface);
     }
-    __syncthreads();
   }
 }
 
@@ -268,7 +235,7 @@ struct FaceBox {
   int lo[3], cnt[3];
 };
 template <int N, int RECON, class G, int DIR>
-__global__ void __launch_bounds__(FB, G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN)
+__global__ void __launch_bounds__(FB, G::flat ? FLUX_MINB : FLUX_MINB_GEN)
 face_box_kernel(const __grid_constant__ GridView gv, const __grid_constant__ FaceBox bx,
                 const double *__restrict__ PE, double *__restrict__ Fface, double *__restrict__ cface) {
   const long long t = (long long)blockIdx.x * FB + threadIdx.x;
@@ -576,17 +543,11 @@ __device__ __noinline__ void stage_const_replay(const GridView &gv, const double
   for (int v = 0; v < 4; v++) sp_loc[v] = s_[v];
 }
 
-#ifndef GRIM_SC_MINB
-#define GRIM_SC_MINB 4
-#endif
-#ifndef GRIM_SC_TILED_GEN
-#define GRIM_SC_TILED_GEN 1  // general metric: tiled (TMA) stage-constant kernel as well
-#endif
-#ifndef GRIM_SC_MINB_GEN
-#define GRIM_SC_MINB_GEN 2  // general metric: connection contractions, 6 neighbour geometries -> 255 registers
-#endif
+// resident blocks per SM of the stage-constant kernels; general metric: connection contractions and 6 neighbour
+// geometries need 255 registers -> 2
+static constexpr int SC_MINB = 4, SC_MINB_GEN = 2;
 template <int N, class G, bool CT>
-__global__ void __launch_bounds__(FB, G::flat ? GRIM_SC_MINB : GRIM_SC_MINB_GEN)
+__global__ void __launch_bounds__(FB, G::flat ? SC_MINB : SC_MINB_GEN)
 stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE,
                    const double *__restrict__ Pn, double dt_stage, const double *__restrict__ Fface,
                    const double *__restrict__ cface, double *__restrict__ C, double *__restrict__ Gx,
@@ -635,7 +596,7 @@ stage_const_kernel(const __grid_constant__ GridView gv, const double *__restrict
 // thread consumed by a serial sum.  Used for Minkowski grids with X^2 active (2.40 -> 2.28 ms at 256^3); the untiled
 // kernel serves 1-D grids, general metrics and the dt probe (which also reduces the face speeds).
 template <int N, class G, bool CT>
-__global__ void __launch_bounds__(FB, G::flat ? GRIM_SC_MINB : GRIM_SC_MINB_GEN)
+__global__ void __launch_bounds__(FB, G::flat ? SC_MINB : SC_MINB_GEN)
 stage_const_tiled_kernel(const __grid_constant__ GridView gv, const double *__restrict__ PE,
                          const double *__restrict__ Pn, double dt_stage, const double *__restrict__ Fface,
                          const double *__restrict__ cface, double *__restrict__ C, double *__restrict__ Gx) {
@@ -726,7 +687,7 @@ struct FluxMaps {
 };
 
 template <int N, class G, bool CT>
-__global__ void __launch_bounds__(FB, G::flat ? GRIM_SC_MINB : GRIM_SC_MINB_GEN)
+__global__ void __launch_bounds__(FB, G::flat ? SC_MINB : SC_MINB_GEN)
 stage_const_tma_kernel(const __grid_constant__ GridView gv, const __grid_constant__ FluxMaps maps,
                        const double *__restrict__ PE, const double *__restrict__ Pn, double dt_stage,
                        const double *__restrict__ Fface, const double *__restrict__ cface, double *__restrict__ C,
@@ -837,8 +798,7 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
     auto tiles = [&](int t0, int t1, int t2) {
       return dim3((unsigned)((f0 + t0 - 1) / t0), (unsigned)((f1 + t1 - 1) / t1), (unsigned)((f2 + t2 - 1) / t2));
     };
-    bool by_tma = false;
-#if GRIM_FLUX_TMA
+    bool by_tma = false;   // false: no tensor map for this array (odd X^1 extent: rows not 16-byte aligned) -> staging kernels
     {
       auto tma = [&](auto dirc) {
         constexpr int D = decltype(dirc)::value;
@@ -848,21 +808,17 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
         if (!make_tile_map(&map, PE, gv.sz[0], gv.sz[1], gv.sz[2], N, gv.zg, X::E0, X::E1, X::E2)) return false;
         const dim3 tg = tiles(T::T0, T::T1, T::T2);
         const long long nt = (long long)tg.x * tg.y * tg.z;
-        const size_t smem = (GRIM_FLUX_TMA_WAVES == 0 ? 1 : 2) * tma_tile_bytes<N, RECON, D>();
+        const size_t smem = tma_tile_bytes<N, RECON, D>();
         auto kern = face_flux_tma_kernel<N, RECON, G, D>;
         cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        const int per_sm = G::flat ? GRIM_FLUX_MINB : GRIM_FLUX_MINB_GEN;
-        long long blocks = (long long)per_sm * (gv.nsm > 0 ? gv.nsm : 148) * GRIM_FLUX_TMA_WAVES;
-        if (blocks > nt || GRIM_FLUX_TMA_WAVES == 0) blocks = nt;
         if (nt >= (1LL << 31)) return false;
-        kern<<<(unsigned)blocks, FB, smem, s>>>(gv, map, PE, Fa, ca, (int)tg.x, (int)tg.y, (int)tg.z);
+        kern<<<(unsigned)nt, FB, smem, s>>>(gv, map, PE, Fa, ca, (int)tg.x, (int)tg.y);
         return true;
       };
       if (a == 0) by_tma = tma(std::integral_constant<int, 0>());
       if (a == 1) by_tma = tma(std::integral_constant<int, 1>());
       if (a == 2) by_tma = tma(std::integral_constant<int, 2>());
     }
-#endif
     if (!by_tma) {
       if (a == 0) face_flux_kernel<N, RECON, G, 0><<<tiles(128, 1, 1), FB, 0, s>>>(gv, PE, Fa, ca);
       if (a == 1) face_flux_kernel<N, RECON, G, 1><<<tiles(32, 4, 1), FB, 0, s>>>(gv, PE, Fa, ca);
@@ -917,10 +873,9 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
   }
   if (!(what & 2)) return launches;
   const unsigned blocks = (unsigned)((gv.nint + FB - 1) / FB);
-  if (!cnt && gv.ngd[1] > 0 && (G::flat || GRIM_SC_TILED_GEN)) {
+  if (!cnt && gv.ngd[1] > 0) {
     const dim3 tg((unsigned)((gv.n[0] + 31) / 32), (unsigned)((gv.n[1] + 3) / 4), (unsigned)gv.n[2]);
     bool by_tma = false;
-#if GRIM_FLUX_TMA
     {
       using TF = TileFluxTma<N, 32, 4>;
       FluxMaps maps;
@@ -946,7 +901,6 @@ static int launch_fluxes_t(const GridView &gv, const double *PE, const double *P
         by_tma = true;
       }
     }
-#endif
     if (by_tma) {
     } else if (gv.flux_ct) stage_const_tiled_kernel<N, G, true><<<tg, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx);
     else stage_const_tiled_kernel<N, G, false><<<tg, FB, 0, s>>>(gv, PE, Pn, dt_stage, Fface, cface, C, Gx);

@@ -7,10 +7,7 @@
 
 namespace grim {
 
-#ifndef GRIM_NB
-#define GRIM_NB 128
-#endif
-static constexpr int NB = GRIM_NB;  // threads per block; 2 blocks/SM: 2 x 128 x (N*N*8 B) of Jacobian + 255 registers
+static constexpr int NB = 128;  // threads per block; 2 blocks/SM: 2 x 128 x (N*N*8 B) of Jacobian + 255 registers
 
 struct StageArgs {
   const double *Pn, *PE, *C, *Gx;
@@ -36,7 +33,7 @@ __device__ __forceinline__ int stage_zone(A &ar, const GridView &gv, const Stage
                                           int st, double *sj) {
   constexpr int M = Unknowns<N, RED>::M;
   // EMHD full solve: the constants of the q / dP rows go to the unused words of the Jacobian's B rows
-  constexpr bool KSM = GRIM_KSM && N == 10 && use_structure<N, RED>();
+  constexpr bool KSM = N == 10 && use_structure<N, RED>();
   static_assert(!KSM || K_COUNT <= 3 * (N - 1), "constants do not fit the free Jacobian words");
   StageProblem<N, G, NB, KSM> prob;
   prob.m = gv.m;
@@ -101,12 +98,9 @@ __device__ __noinline__ int stage_zone_replay(const GridView &gv, const StageArg
   return stage_zone<N, G, RED, APPEND>(ar, gv, a, z, i, j, st, sj);
 }
 
-#ifndef GRIM_N8_MINB
-#define GRIM_N8_MINB 2  // ideal MHD: 64 + 8 doubles of shared memory per zone would allow 3 blocks (170 registers)
-#endif
-#ifndef GRIM_RED_MINB
-#define GRIM_RED_MINB 2  // reduced solve: (N-3)^2 + N doubles of shared memory per zone leave room for 3 blocks
-#endif
+// Resident blocks per SM.  Ideal MHD (64 + 8 doubles of shared memory per zone) and the reduced solve ((N-3)^2 + N) would
+// have room for 3 blocks at 170 registers; 2 at 255 registers measured faster.
+static constexpr int N8_MINB = 2, RED_MINB = 2;
 // One thread's zone of a launch: interior zone zt (have = false: the thread has none).  Returns the packed result of
 // stage_zone with the deferred zones appended to a.next_list and removed from the count.
 template <int N, class G, bool RED, bool APPEND>
@@ -139,7 +133,7 @@ __device__ __forceinline__ int stage_thread(const GridView &gv, const StageArgs 
 
 // APPEND: first sweep (zones that stop at the lowered kmax are deferred to a.next_list)
 template <int N, class G, bool RED, bool APPEND>
-__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB))
+__global__ void __launch_bounds__(NB, RED ? RED_MINB : (N == 8 ? N8_MINB : 256 / NB))
 newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
@@ -156,7 +150,7 @@ newton_stage_kernel(const __grid_constant__ GridView gv, const __grid_constant__
 // The launch over a list of deferred zones whose length is on the device (cnt->list_count, written by the launch
 // before): a resident grid of blocks strides over the list, so that the host need not know the length.
 template <int N, class G, bool RED>
-__global__ void __launch_bounds__(NB, RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB))
+__global__ void __launch_bounds__(NB, RED ? RED_MINB : (N == 8 ? N8_MINB : 256 / NB))
 newton_stage_list_kernel(const __grid_constant__ GridView gv, const __grid_constant__ StageArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long nlist = (long long)cnt->list_count;
@@ -188,7 +182,7 @@ static int launch_stage_t(const GridView &gv, const double *Pn, const double *PE
   if (list) {
     // the list's length is cnt->list_count on the device: a resident grid strides over it (nothing to do: ~5 us)
     cudaFuncSetAttribute(newton_stage_list_kernel<N, G, RED>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    const int per_sm = RED ? GRIM_RED_MINB : (N == 8 ? GRIM_N8_MINB : 256 / NB);
+    const int per_sm = RED ? RED_MINB : (N == 8 ? N8_MINB : 256 / NB);
     newton_stage_list_kernel<N, G, RED><<<(unsigned)(per_sm * (gv.nsm > 0 ? gv.nsm : 148)), NB, smem, s>>>(gv, a, cnt);
     return 1;
   }
@@ -283,7 +277,7 @@ __device__ __noinline__ int invert_zone_replay(const GridView &gv, const InvertA
 }
 
 template <int N, class G>
-__global__ void __launch_bounds__(NB, N == 8 ? GRIM_N8_MINB : 256 / NB)
+__global__ void __launch_bounds__(NB, N == 8 ? N8_MINB : 256 / NB)
 invert_kernel(const __grid_constant__ GridView gv, const __grid_constant__ InvertArgs a, Counters *cnt) {
   extern __shared__ double smem[];
   const long long t = (long long)blockIdx.x * NB + threadIdx.x;
@@ -397,7 +391,7 @@ static __device__ __align__(256) unsigned char static_scratch[STATIC_SCRATCH_BYT
 // invert_kernel with 32-bit lists at caller-supplied addresses (the host passes addresses inside static_scratch).
 // Zones are solved by the same invert_zone as the allocating path, so a zone's result is the same bits.
 template <int N, class G>
-__global__ void __launch_bounds__(NB, N == 8 ? GRIM_N8_MINB : 256 / NB)
+__global__ void __launch_bounds__(NB, N == 8 ? N8_MINB : 256 / NB)
 invert_static_kernel(const __grid_constant__ GridView gv, const __grid_constant__ InvertArgs a, Counters *cnt,
                      const uint32_t *__restrict__ list, uint32_t *__restrict__ next_list) {
   extern __shared__ double smem[];

@@ -115,12 +115,9 @@ __host__ __device__ constexpr bool jac_zero(int row, int col) {
   if (row >= QQ) return (col >= B1 && col <= B3) || (col >= QQ && col != row);
   return false;
 }
-#ifndef GRIM_JAC_STRUCT
-#define GRIM_JAC_STRUCT 1
-#endif
 // full solves of both problems use the structure; the reduced solve has no B rows and keeps the general path
 template <int N, bool RED>
-__host__ __device__ constexpr bool use_structure() { return GRIM_JAC_STRUCT && !RED; }
+__host__ __device__ constexpr bool use_structure() { return !RED; }
 
 __device__ __forceinline__ double zero_times(double ih) {  // (+0) * ih for finite ih
   return __hiloint2double(__double2hiint(ih) & 0x80000000, 0);
@@ -144,7 +141,7 @@ __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverP
 #pragma unroll
   for (int i = 0; i < U::M; i++) {
     const int row = U::prim(i);
-    if (GRIM_JAC_STRUCT && jac_zero<N>(row, J)) {
+    if (jac_zero<N>(row, J)) {
       if (!(STRUCT && row >= B1 && row <= B3)) jac.at(JacView<U::M, BLOCK>::row(i), S) = zero_times(ih);
     } else {
       jac.at(JacView<U::M, BLOCK>::row(i), S) = (Rt[row] - R0[row]) * ih;
@@ -156,26 +153,15 @@ __device__ __forceinline__ void fd_column(A &ar, const Prob &prob, const SolverP
 // state (q, dP), then the thermodynamic ones (reuse velocity, field, bhat), the field ones (velocity, thermo), last
 // the velocity ones (thermo only) -- so the cached pieces die as early as possible and the later, more expensive
 // columns have the registers.  The Jacobian does not depend on the order.
-#ifndef GRIM_FD_ORDER
-#define GRIM_FD_ORDER 1
-#endif
 template <int N, bool RED>
 __host__ __device__ constexpr int fd_order(int s) {
   if (RED) {  // unknown indices: rho u u~1 u~2 u~3 (q dP)
     constexpr int red10[7] = {5, 6, 0, 1, 2, 3, 4};
     return N == 10 ? red10[s] : s;
   }
-#if GRIM_FD_ORDER == 1
   constexpr int ord10[10] = {QQ, DPP, RHO, UU, B1, B2, B3, U1, U2, U3};
   constexpr int ord8[8] = {RHO, UU, B1, B2, B3, U1, U2, U3};
   return N == 10 ? ord10[s] : ord8[s];
-#elif GRIM_FD_ORDER == 2
-  constexpr int ord10[10] = {U1, U2, U3, B1, B2, B3, RHO, UU, QQ, DPP};
-  constexpr int ord8[8] = {U1, U2, U3, B1, B2, B3, RHO, UU};
-  return N == 10 ? ord10[s] : ord8[s];
-#else
-  return s;
-#endif
 }
 
 template <int S, int N, bool RED, int BLOCK, class A, class Prob, bool DONE = (S == Unknowns<N, RED>::M)>
@@ -272,7 +258,7 @@ __device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, do
 // The same factorisation by register panels.  Shared memory moves 128 B per cycle and SM -- a warp's 8-byte
 // load costs as much as four of its fp64 instructions -- and the column-at-a-time LU above loads every
 // multiplier once per later column (285 loads for N = 10): the solve was bound by the shared-memory pipe
-// (profiles/r2a_newton_lu_panels.md).  Here a panel of columns is held in registers at a time: the multipliers
+// (DESIGN.md 13.2).  Here a panel of columns is held in registers at a time: the multipliers
 // of the earlier pivots are loaded once per panel, those of the panel's own pivots are never loaded, and the
 // last panel carries the right-hand side along and is never stored -- the back substitution reads its U from
 // the registers.  N = 10 with panels of 5 + 5 columns loads 35 multipliers; N <= 8 is one panel (no stores).
@@ -347,105 +333,6 @@ __device__ __forceinline__ void lu_panel(A &ar, const JacView<M, BLOCK> &jac, in
   }
 }
 
-// Panel split of the M x M solve.  N = 10: cuts from GRIM_LU_CUTS; smaller systems (ideal MHD, reduced solves,
-// 8 x 8 and below) are one panel, i.e. factorised entirely in registers.
-// GRIM_LU_CUTS: the decimal digits are the interior cuts, ascending (4 -> panels [0,4) [4,10); 2468 -> pairs).
-#ifndef GRIM_LU_CUTS
-#define GRIM_LU_CUTS 4
-#endif
-template <int M>
-struct LuSplit {
-  static constexpr int n = 1;
-  static __host__ __device__ constexpr int b(int) { return 0; }
-  static __host__ __device__ constexpr int e(int) { return M; }
-};
-__host__ __device__ constexpr int lu_cut_count() {
-  int c = 0;
-  for (long long v = GRIM_LU_CUTS; v > 0; v /= 10) c++;
-  return c;
-}
-// boundary q (0 .. count + 1): 0, the digits, 10
-__host__ __device__ constexpr int lu_cut(int q) {
-  if (q <= 0) return 0;
-  if (q > lu_cut_count()) return 10;
-  long long v = GRIM_LU_CUTS;
-  for (int s = 0; s < lu_cut_count() - q; s++) v /= 10;
-  return (int)(v % 10);
-}
-template <>
-struct LuSplit<10> {
-  static constexpr int n = lu_cut_count() + 1;
-  static __host__ __device__ constexpr int b(int pi) { return lu_cut(pi); }
-  static __host__ __device__ constexpr int e(int pi) { return lu_cut(pi + 1); }
-};
-
-// Panel PI and all later ones; the last panel carries b along, is not stored, and ends with the back substitution.
-template <int M, int BLOCK, int PI, class A>
-__device__ __forceinline__ void lu_panels_from(A &ar, const JacView<M, BLOCK> &jac, int (&rowoff)[M], double (&b)[M],
-                                               bool &ok) {
-  using S = LuSplit<M>;
-  constexpr int C0 = S::b(PI), C1 = S::e(PI), CB = C1 - C0;
-  constexpr bool LAST = (PI == S::n - 1);
-  double X[CB][M], rinv[CB];
-  // the panel's columns in pivoted order (the identity for the first panel)
-#pragma unroll
-  for (int c = 0; c < CB; c++)
-#pragma unroll
-    for (int i = 0; i < M; i++)
-      X[c][i] = (C0 == 0) ? jac.at(JacView<M, BLOCK>::row(i), C0 + c) : jac.at(rowoff[i], C0 + c);
-  if (LAST && C0 > 0) {
-    // b into pivoted order through the storage of the last column, which the loads have just emptied
-#pragma unroll
-    for (int i = 0; i < M; i++) jac.at(JacView<M, BLOCK>::row(i), M - 1) = b[i];
-#pragma unroll
-    for (int i = 0; i < M; i++) b[i] = jac.at(rowoff[i], M - 1);
-  }
-  // updates of the earlier panels' pivots, k ascending
-#pragma unroll
-  for (int k = 0; k < C0; k++) {
-#pragma unroll
-    for (int i = k + 1; i < M; i++) {
-      const double l = jac.at(rowoff[i], k);
-#pragma unroll
-      for (int c = 0; c < CB; c++) X[c][i] = X[c][i] - l * X[c][k];
-      if (LAST) b[i] = b[i] - l * b[k];
-    }
-  }
-  lu_panel<M, BLOCK, C0, CB, LAST, !LAST>(ar, jac, rowoff, X, b, rinv, ok);
-  if constexpr (!LAST) {
-    lu_panels_from<M, BLOCK, PI + 1>(ar, jac, rowoff, b, ok);
-  } else {
-    // back substitution: U of this panel from the registers, U of the earlier ones from shared memory
-#pragma unroll
-    for (int i = M - 1; i >= 0; i--) {
-      double s = b[i];
-#pragma unroll
-      for (int j = i + 1; j < M; j++) {
-        const int jc = j >= C0 ? j - C0 : 0;
-        if (j >= C0) s = s - X[jc][i] * b[j];
-        else s = s - jac.at(rowoff[i], j) * b[j];
-      }
-      const int ic = i >= C0 ? i - C0 : 0;
-      if (i >= C0) b[i] = s * rinv[ic];
-      else b[i] = s * jac.at(rowoff[i], i);
-    }
-  }
-}
-
-template <int M, int BLOCK, class A>
-__device__ __forceinline__ bool lu_solve_panels(A &ar, const JacView<M, BLOCK> &jac, double (&b)[M]) {
-  int rowoff[M];
-#pragma unroll
-  for (int i = 0; i < M; i++) rowoff[i] = JacView<M, BLOCK>::row(i);
-  bool ok = true;
-  lu_panels_from<M, BLOCK, 0>(ar, jac, rowoff, b, ok);
-  return ok;
-}
-
-#ifndef GRIM_LU_PANELS
-#define GRIM_LU_PANELS 0
-#endif
-
 // ---------------------------------------------------------------------------------------------------------
 // The factorisation of the full N x N Jacobian with its structure (jac_zero) used.  The B rows are zero in the
 // columns of rho, u, u~^i, so in the elimination steps k = 0..4 they are never the pivot (a zero is never the
@@ -462,14 +349,11 @@ __device__ __forceinline__ bool lu_solve_panels(A &ar, const JacView<M, BLOCK> &
 // Every element receives the same updates in the same order as in og_lu_solve / lu_solve except those skipped
 // no-ops, which can change nothing but the sign of an exact zero.
 // ---------------------------------------------------------------------------------------------------------
-#ifndef GRIM_LU_GROUP
-#define GRIM_LU_GROUP 5
-#endif
 template <int N, int BLOCK, class A>
 __device__ __forceinline__ bool lu_solve_structured(A &ar, const JacView<N, BLOCK> &jac, double (&b)[N]) {
   constexpr int NA = N - 3;   // active rows
   constexpr int NT = N - 5;   // trailing block
-  constexpr int G = GRIM_LU_GROUP;
+  constexpr int G = 5;   // columns of block B updated per load of the multipliers (1, 2 and 5 measured: 5)
   int ro[NA];
   double ba[NA];
 #pragma unroll
@@ -629,11 +513,7 @@ __device__ __forceinline__ double newton_zone(A &ar, const Prob &prob, const Sol
     if constexpr (use_structure<N, RED>()) {
       ok = lu_solve_structured<M, BLOCK>(ar, jac, dP);
     } else {
-#if GRIM_LU_PANELS
-      ok = lu_solve_panels<M, BLOCK>(ar, jac, dP);
-#else
       ok = lu_solve<M, BLOCK>(ar, jac, dP);
-#endif
     }
     if (singular || !ok) {
       st |= ST_SINGULAR;

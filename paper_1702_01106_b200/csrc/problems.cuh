@@ -25,9 +25,6 @@ __host__ __device__ constexpr int kslot(int i) {
   const int r = B1 + i / (N - 1), c = i % (N - 1);
   return r * N + (c < r ? c : c + 1);
 }
-#ifndef GRIM_KSM
-#define GRIM_KSM 1
-#endif
 
 // CS: stride (in doubles) of the per-thread shared-memory vector that holds the stage constant C
 template <int N, class G, int CS, bool KSM = false>
