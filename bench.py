@@ -46,7 +46,7 @@ NCU_TRAFFIC_SOURCE = "profiles/r2c_final_kernels.md"
 # 8(d) "Flux + stage constant, EMHD": P_E 10 (x 1.3-1.5 halo re-read) + P_n 10 in, C 10 + G 3 out -> 320-400 B; the
 # upper figure.  Algorithmic fp64 work: DADD + DMUL + DFMA thread instructions of the same four kernels in the round's
 # capture of the round-1 kernels (3997 per zone-stage: 3 x 1084 face + 744 stage constant; profiles/r2c_final_kernels.md
-# and DESIGN.md 13.3), frozen like the Newton count.
+# and DESIGN.md 15.3), frozen like the Newton count.
 ALG_BYTES_PER_ZONE_STAGE_FLUX = 400.0
 ALG_FP64_INSTR_PER_ZONE_STAGE_FLUX = 3997.0
 NCU_DRAM_BYTES_PER_ZONE_STAGE_FLUX = 1075.0

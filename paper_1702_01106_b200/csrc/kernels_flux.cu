@@ -170,7 +170,7 @@ face_flux_kernel(const __grid_constant__ GridView gv, const double *__restrict__
 // signals the block's mbarrier.  One thread issues the copy; nobody computes addresses or holds staging registers.  (A TMA
 // box row starts on a 16-byte boundary and is a multiple of 16 bytes long: the box starts at the even X^1 index at or
 // below the first stencil zone and has an even X^1 extent.)  One tile per block: with 4 resident blocks per SM the copies
-// of some blocks overlap the arithmetic of others; a persistent, double-buffered form measured slower (DESIGN.md 12).
+// of some blocks overlap the arithmetic of others; a persistent, double-buffered form measured slower (DESIGN.md 12, 15.3).
 template <int RECON, int DIR>
 struct TmaTile {
   using T = FaceTile<DIR>;

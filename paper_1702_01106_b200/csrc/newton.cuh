@@ -258,7 +258,7 @@ __device__ __forceinline__ bool lu_solve(A &ar, const JacView<N, BLOCK> &jac, do
 // The same factorisation by register panels.  Shared memory moves 128 B per cycle and SM -- a warp's 8-byte
 // load costs as much as four of its fp64 instructions -- and the column-at-a-time LU above loads every
 // multiplier once per later column (285 loads for N = 10): the solve was bound by the shared-memory pipe
-// (DESIGN.md 13.2).  Here a panel of columns is held in registers at a time: the multipliers
+// (DESIGN.md 15.2).  Here a panel of columns is held in registers at a time: the multipliers
 // of the earlier pivots are loaded once per panel, those of the panel's own pivots are never loaded, and the
 // last panel carries the right-hand side along and is never stored -- the back substitution reads its U from
 // the registers.  N = 10 with panels of 5 + 5 columns loads 35 multipliers; N <= 8 is one panel (no stores).
